@@ -1,0 +1,292 @@
+"""Pins of the fp64 oracle against what the paper and the mathematics fix (no GPU).
+
+Each test names the PAPER.md passage it rests on.  The pins are chosen so that a dropped
+mirror, a wrong centre/crop offset, a missing root, a transposed axis or a wrong compound
+product fails at least one of them.
+"""
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+import scipy.ndimage as ndi
+import scipy.signal as sps
+
+import mvd_synth
+from oracle import mvd_oracle as O
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+@pytest.fixture(scope="module")
+def tiny():
+    return mvd_synth.make_tiny_asymmetric(dims=(11, 9, 7), psf_dims=(5, 3, 7), n_views=3)
+
+
+# ---- worked example (tests/golden/rl_1d_worked_example.txt; eq. 13) -----------------
+def test_worked_example_eq13():
+    rows = [l.split() for l in open(os.path.join(HERE, "golden", "rl_1d_worked_example.txt"))
+            if l.strip() and not l.startswith("#")]
+    col = lambda i: np.array([float(Fraction(r[i])) for r in rows])
+    phi, p, b, q, f, psi1 = (col(i) for i in range(6))
+    vol = lambda a: a.reshape(1, 1, -1)
+    psi0 = O.initial_estimate([vol(phi)])
+    assert np.allclose(psi0, 8.0)
+    for same in (O.same_direct, O.same_fft):
+        assert np.allclose(same(psi0, vol(p)).ravel(), b, rtol=1e-14)
+        assert np.allclose(same(vol(q), O.flip(vol(p))).ravel(), f, rtol=1e-14)
+    for variant in O.VARIANTS:
+        out = O.deconvolve([vol(phi)], [vol(p)], variant, 1, eps=0.0, psi_floor=0.0)
+        assert np.allclose(out.ravel(), psi1, rtol=1e-13)
+
+
+# ---- P1: brute force == FFT (definition, eq. 3) -----------------------------------
+def test_p1_direct_equals_fft(tiny):
+    rng = np.random.default_rng(1)
+    a = rng.random((7, 9, 11))
+    for p in tiny.psfs:
+        assert np.abs(O.same_direct(a, p) - O.same_fft(a, p)).max() < 1e-13
+        assert np.abs(O.conv_full_direct(a, p) - O.conv_full_fft(a, p)).max() < 1e-13
+
+
+def test_p1_same_matches_library_conventions(tiny):
+    """same() against two library routines that define centring/flip themselves:
+    scipy.signal.convolve(mode='same') and scipy.ndimage.correlate(mode='constant')."""
+    rng = np.random.default_rng(2)
+    a = rng.random((7, 9, 11))
+    p = tiny.psfs[0].astype(np.float64)
+    ref = sps.convolve(a, p, mode="same", method="direct")
+    assert np.abs(O.same_direct(a, p) - ref).max() < 1e-13
+    # convolution with the mirrored kernel is correlation with the kernel (L312)
+    ref2 = ndi.correlate(a, p, mode="constant", cval=0.0)
+    assert np.abs(O.same_direct(a, O.flip(p)) - ref2).max() < 1e-13
+
+
+@pytest.mark.parametrize("variant,mode", [("independent", "auto"), ("efficient", "auto"),
+                                          ("osem", "auto"), ("osem", "plain"), ("efficient", "opt1"),
+                                          ("osem", "opt2")])
+def test_p1_full_iteration_backends_agree(tiny, variant, mode):
+    a = O.deconvolve(tiny.views, tiny.psfs, variant, 2, kernel_mode=mode, backend="direct")
+    b = O.deconvolve(tiny.views, tiny.psfs, variant, 2, kernel_mode=mode, backend="fft")
+    assert np.abs(a - b).max() / np.abs(a).max() < 1e-12
+
+
+# ---- P2: one view == classical RL (L421, L628 W = empty set, L780) ------------------------
+def test_p2_single_view_is_classical_rl(tiny):
+    phi, p = tiny.views[0].astype(np.float64), tiny.psfs[0].astype(np.float64)
+    p = p / p.sum()
+    # classical RL written with library routines only (scipy.ndimage): blur = convolve,
+    # back-projection = correlate with the same kernel (integration over x, L312).
+    psi = np.full(phi.shape, phi.mean())
+    for _ in range(3):
+        b = ndi.convolve(psi, p, mode="constant", cval=0.0)
+        psi = psi * ndi.correlate(phi / b, p, mode="constant", cval=0.0)
+    outs = [O.deconvolve([phi], [p], v, 3, kernel_mode=m)
+            for v in O.VARIANTS for m in ("auto", "plain", "compound", "opt1", "opt2")]
+    for o in outs:
+        assert np.abs(o - psi).max() / psi.max() < 1e-12
+    k = O.back_projector([p], 0, "compound")
+    assert np.abs(k - O.flip(p)).max() < 1e-15
+
+
+# ---- P3: flux identity (eq. 52-55) ----------------------------------------------
+def test_p3_flux_identity_pins_mirror_and_centre(tiny):
+    psi = np.random.default_rng(3).random(tiny.views[0].shape) + 0.5
+    for phi, p in zip(tiny.views, tiny.psfs):
+        p = O.normalise(p)
+        f = O.rl_factor(psi, phi, p, O.flip(p), eps=0.0)
+        assert abs((psi * f).sum() / phi.astype(np.float64).sum() - 1.0) < 1e-12
+        # the un-mirrored kernel must NOT conserve flux on an asymmetric PSF
+        f_bad = O.rl_factor(psi, phi, p, p, eps=0.0)
+        assert abs((psi * f_bad).sum() / phi.astype(np.float64).sum() - 1.0) > 1e-5
+
+
+def test_p3_combined_root_flux_bound(tiny):
+    """eq. 56-62 (AM >= GM): sum psi_new <= mean_v sum phi_v for the rooted combined update."""
+    o = O.Oracle(tiny.views, tiny.psfs, "independent")
+    bound = np.mean([v.astype(np.float64).sum() for v in tiny.views])
+    for _ in range(4):
+        o.iterate(1)
+        assert o.psi.sum() <= bound * (1 + 1e-12)
+    assert o.flux == pytest.approx(o.psi.sum(), rel=1e-15)
+
+
+# ---- P4: fixed point (L306) ---------------------------------------------------------------
+def test_p4_fixed_point(tiny):
+    rng = np.random.default_rng(4)
+    shape = (15, 13, 17)
+    star = rng.random(shape) + 1.0
+    psfs = [O.normalise(p) for p in tiny.psfs]
+    views = [O.same_fft(star, p) for p in psfs]
+    rz, ry, rx = 3, 1, 2            # PSF half sizes for box (Kx,Ky,Kz) = (5,3,7)
+    for mode in ("plain", "compound", "opt1", "opt2"):
+        for v in range(3):
+            k = O.back_projector(psfs, v, mode)
+            f = O.rl_factor(star, views[v], psfs[v], k, eps=0.0)
+            inner = f[rz:-rz, ry:-ry, rx:-rx]
+            assert np.abs(inner - 1.0).max() < 1e-12          # interior: f == 1
+            assert np.abs(f - O.same_direct(np.ones(shape), k)).max() < 1e-12   # closed form
+            assert f.min() < 0.9                               # faces are darkened (R3 ii)
+
+
+# ---- P5: identical views (L847) -----------------------------------------------------------
+def test_p5_identical_views(tiny):
+    phi, p = tiny.views[1], tiny.psfs[1]
+    one = O.deconvolve([phi], [p], "independent", 3)
+    four = O.deconvolve([phi] * 4, [p] * 4, "independent", 3)
+    assert np.abs(one - four).max() / one.max() < 1e-12
+    # OSEM with plain kernels and V copies = V single-view iterations per iteration
+    osem = O.deconvolve([phi] * 4, [p] * 4, "osem", 1, kernel_mode="plain")
+    rl4 = O.deconvolve([phi], [p], "osem", 4, kernel_mode="plain")
+    assert np.abs(osem - rl4).max() / rl4.max() < 1e-12
+    # and the literal product (eq. 38 as printed) is NOT one view: it takes V unit steps at once
+    lit = O.deconvolve([phi] * 4, [p] * 4, "independent", 1, literal_product=True)
+    assert np.abs(lit - O.deconvolve([phi], [p], "independent", 1)).max() / one.max() > 1e-3
+
+
+# ---- P6: delta PSF (L851) -----------------------------------------------------------------
+def test_p6_delta_psf(tiny):
+    delta = np.zeros((7, 3, 5))
+    delta[3, 1, 2] = 1.0
+    views = [v.astype(np.float64) + 1.0 for v in tiny.views]
+    for mode in ("plain", "compound", "opt1", "opt2"):
+        k = O.back_projector([delta] * 3, 0, mode)
+        assert np.abs(k - delta).max() < 1e-15
+    assert np.allclose(O.deconvolve(views[:1], [delta], "osem", 1), views[0], rtol=1e-14)
+    assert np.allclose(O.deconvolve(views, [delta] * 3, "osem", 1), views[-1], rtol=1e-14)
+    gm = (views[0] * views[1] * views[2]) ** (1.0 / 3.0)
+    assert np.allclose(O.deconvolve(views, [delta] * 3, "efficient", 1), gm, rtol=1e-13)
+
+
+# ---- P7: compound kernel of Gaussians, closed form (eq. 105 + Gaussian algebra) --------------
+def _cov(sxy, sz, deg):
+    t = np.radians(deg)
+    c, s = np.cos(t), np.sin(t)
+    r = np.array([[c, 0, s], [0, 1, 0], [-s, 0, c]])
+    return r @ np.diag([sxy ** 2, sxy ** 2, sz ** 2]) @ r.T
+
+
+def _gauss_box(cov, box):
+    kx, ky, kz = box
+    uz, uy, ux = np.meshgrid(np.arange(kz) - kz // 2, np.arange(ky) - ky // 2, np.arange(kx) - kx // 2,
+                             indexing="ij")
+    u = np.stack([ux, uy, uz], -1).astype(float)
+    g = np.exp(-0.5 * np.einsum("...i,ij,...j->...", u, np.linalg.inv(cov), u))
+    return g / g.sum()
+
+
+@pytest.mark.parametrize("mode", ["compound", "opt1"])
+def test_p7_compound_gaussian_closed_form(mode):
+    box = (27, 27, 27)
+    angles = (0.0, 50.0, 100.0, 150.0)
+    covs = [_cov(1.6, 2.6, a) for a in angles]
+    psfs = [_gauss_box(c, box) for c in covs]
+    for v in range(len(covs)):
+        k = O.back_projector(psfs, v, mode)
+        lam = np.linalg.inv(covs[v])
+        for w in range(len(covs)):
+            if w != v:
+                # Gaussian * Gaussian adds covariances; pointwise product adds precisions
+                lam = lam + np.linalg.inv(covs[v] + (2 if mode == "compound" else 1) * covs[w])
+        ref = _gauss_box(np.linalg.inv(lam), box)
+        assert np.linalg.norm(k - ref) / np.linalg.norm(ref) < 2e-6
+    # a mistake such as leaving out P_w* or the P_v* factor is visible at this tolerance
+    wrong = O.back_projector(psfs, 0, "opt1" if mode == "compound" else "compound")
+    lam = np.linalg.inv(covs[0]) + sum(np.linalg.inv(covs[0] + (2 if mode == "compound" else 1) * covs[w])
+                                       for w in (1, 2, 3))
+    assert np.linalg.norm(wrong - _gauss_box(np.linalg.inv(lam), box)) > 1e-3 * np.linalg.norm(wrong)
+
+
+def test_opt2_is_power_of_mirrored_psf(tiny):
+    psfs = [O.normalise(p) for p in tiny.psfs]
+    k = O.back_projector(psfs, 2, "opt2")
+    ref = O.flip(psfs[2]) ** 3
+    assert np.abs(k - ref / ref.sum()).max() < 1e-16
+
+
+def test_compound_is_asymmetric_product_on_psf_box(tiny):
+    """eq. 105 on non-symmetric PSFs, written out tap by tap (triple sum over offsets measured
+    from each kernel's centre) for two output taps; k is normalised, so compare their ratio."""
+    psfs = [O.normalise(p) for p in tiny.psfs]
+    k = O.back_projector(psfs, 0, "compound", backend="direct")
+    pvs = O.flip(psfs[0])
+    c = tuple(n // 2 for n in pvs.shape)
+
+    def t_vw(pw, u):                                    # (P_v* * P_w * P_w*)(u - c)
+        pws = O.flip(pw)
+        tot = 0.0
+        for a in np.ndindex(pvs.shape):
+            for b in np.ndindex(pw.shape):
+                idx = tuple((u[i] - c[i]) - (a[i] - c[i]) - (b[i] - c[i]) + c[i] for i in range(3))
+                if all(0 <= idx[i] < pws.shape[i] for i in range(3)):
+                    tot += pvs[a] * pw[b] * pws[idx]
+        return tot
+
+    def tap(u):
+        return pvs[u] * t_vw(psfs[1], u) * t_vw(psfs[2], u)
+
+    u1, u2 = (1, 2, 0), c
+    assert k[u1] / k[u2] == pytest.approx(tap(u1) / tap(u2), rel=1e-12)
+
+
+# ---- P8: monotone likelihood (eq. 39-43) --------------------------------------------
+def test_p8_likelihood_monotone(tiny):
+    """The proof needs sum_x P(x|xi) = 1 wherever psi* > 0 (Jensen, eq. 46-47) and equal view
+    integrals (eq. 62): psi* supported >= r away from the faces, noise-free views."""
+    rng = np.random.default_rng(8)
+    shape = (19, 11, 15)
+    star = np.zeros(shape)
+    star[3:-3, 1:-1, 2:-2] = rng.random((13, 9, 11)) ** 3 * 50 + 0.1
+    psfs = [O.normalise(p) for p in tiny.psfs]
+    views = [O.same_fft(star, p) for p in psfs]
+    for v in views:
+        assert v.sum() == pytest.approx(star.sum(), rel=1e-13)
+    mask = star > 0
+    for kernel_mode in ("plain",):
+        o = O.Oracle(views, psfs, "independent", kernel_mode=kernel_mode, eps=0.0, psi_floor=0.0)
+        last = -np.inf
+        for _ in range(15):
+            o.iterate(1)
+            l = float(-(star[mask] * np.log(star[mask] / o.psi[mask])).sum())     # eq. 39
+            assert l >= last - 1e-9
+            assert o.psi.sum() <= star.sum() * (1 + 1e-12)                         # eq. 56
+            last = l
+    # without the root the printed product of eq. 38 does not keep eq. 56
+    lit = O.Oracle(views, psfs, "independent", literal_product=True, eps=0.0, psi_floor=0.0)
+    lit.iterate(3)
+    assert lit.psi.sum() > star.sum() * 1.01 or not np.isfinite(lit.psi).all()
+
+
+# ---- P9: ordering of the variants (L807-809) -------------------------------------------------
+def test_p9_variant_ordering():
+    prob = mvd_synth.make_problem(2, dims=(40, 36, 32), psf_dims=(9, 9, 17), noise=False)
+    gt = prob.gt.astype(np.float64)
+    inner = (slice(8, -8), slice(4, -4), slice(4, -4))
+    err = {}
+    for variant in O.VARIANTS:
+        o = O.Oracle(prob.views, prob.psfs, variant)
+        e = []
+        for _ in range(6):
+            o.iterate(1)
+            e.append(O.average_difference(o.psi[inner], gt[inner]))
+        assert all(b < a for a, b in zip(e, e[1:])), variant      # every variant improves
+        err[variant] = e[-1]
+    assert err["osem"] < err["efficient"] < err["independent"]
+
+
+# ---- blocks (L64, L943; R13) -----------------------------------------------------------------
+def test_blocked_equals_whole_when_one_block(tiny):
+    whole = O.deconvolve(tiny.views, tiny.psfs, "osem", 2)
+    blk = O.deconvolve_blocked(tiny.views, tiny.psfs, tiny.views[0].shape, "osem", 2)
+    assert np.abs(whole - blk).max() / whole.max() < 1e-13
+
+
+def test_blocked_is_close_to_whole_in_block_interiors():
+    prob = mvd_synth.make_problem(1, dims=(32, 32, 32), psf_dims=(5, 5, 9), n_views=2)
+    whole = O.deconvolve(prob.views, prob.psfs, "osem", 1)
+    blk = O.deconvolve_blocked(prob.views, prob.psfs, (16, 16, 16), "osem", 1, halo_zyx=(8, 4, 4))
+    # halo = 2r: after ONE osem iteration of 2 views the dependence radius is 2 views x 2 convs x r,
+    # so only block centres agree closely; the blocked mode is an approximation (L943)
+    rel = np.abs(whole - blk) / np.maximum(whole, 1e-6)
+    assert np.median(rel) < 1e-2
+    assert blk.shape == whole.shape and np.isfinite(blk).all()
