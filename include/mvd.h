@@ -1,0 +1,163 @@
+/* mvd.h -- C ABI of the B200 multi-view Richardson-Lucy deconvolution library (libmvd.so).
+ *
+ * What the library computes (citations are PAPER.md lines of arXiv 1308.0730, "Efficient
+ * Bayesian-based Multi-View Deconvolution"; "R<n>" are the readings listed in DESIGN.md):
+ *
+ *   For every view v of V registered views phi_v with point spread function P_v
+ *       b_v   = psi (*) P_v                               expected image     (eq. 1, eq. 13)
+ *       q_v   = phi_v / max(b_v, eps)                     quotient           (L306; clamp R4)
+ *       f_v   = q_v (*) K_v                               back-projection    (eq. 70, eq. 104)
+ *   with (*) the linear convolution, zero extension outside the volume, output cropped to the
+ *   volume (R3), and K_v the back-projector:
+ *       PLAIN     K_v = P_v*  (mirrored PSF, L312)                            eq. 70
+ *       COMPOUND  K_v = P_v* . prod_{w!=v} crop(P_v* (*) P_w (*) P_w*)        eq. 105
+ *       OPT1      K_v = P_v* . prod_{w!=v} crop(P_v* (*) P_w)                 eq. 107
+ *       OPT2      K_v = (P_v*)^V                                              eq. 108 L751-758 (R9)
+ *   (pointwise products on the box of P_v, centre aligned, renormalised to sum 1: R5, R6).
+ *   The estimate is then updated
+ *       MVD_OSEM         psi <- max(psi * f_v, psi_floor) after every view, v = 0..V-1   (eq. 109-112)
+ *       MVD_INDEPENDENT  psi <- max(psi * (prod_v max(f_v,0))^(1/V), psi_floor), K = PLAIN     (eq. 70; root: eq. 44, R1)
+ *       MVD_EFFICIENT    same combination, K = COMPOUND                                        (eq. 104)
+ *   One iteration = every view has contributed once (footnote L817).
+ *
+ * Memory conventions
+ *   - Volumes are fp32, x fastest: element (x,y,z) at [(z*Ny + y)*Nx + x].  dims = {Nx,Ny,Nz}.
+ *   - `views` are DEVICE pointers; they are BORROWED (read-only, never copied) and must stay valid
+ *     and unchanged until mvd_destroy.
+ *   - `psfs` are HOST pointers, x fastest, dims psf_dims[v] = {Kx,Ky,Kz}, all odd, K <= N per axis,
+ *     values >= 0 with a positive sum (eq. 4).  They are copied during mvd_create.
+ *   - ALL device memory the library uses is the caller's `workspace` (device pointer, at least
+ *     mvd_workspace_size bytes, 256-byte aligned).  It must outlive the context.  The estimate psi
+ *     lives inside it.  The library itself allocates no device memory.
+ *   - `stream` is a cudaStream_t (as void*); NULL = the legacy default stream.  Every call enqueues
+ *     its work on that stream; mvd_iterate is asynchronous.  Calls that return data to the HOST
+ *     synchronise the stream.
+ * Errors: every call returns an mvd_status, never throws or aborts.  On failure mvd_create sets
+ *   *out = NULL.  A CUDA error is sticky: later calls on the context return MVD_ERR_STATE.
+ * Threading: one context per stream; calls on one context are not re-entrant.
+ */
+#ifndef MVD_H_
+#define MVD_H_
+
+#include <stddef.h>
+
+#if defined(__GNUC__)
+#define MVD_API __attribute__((visibility("default")))
+#else
+#define MVD_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mvd_ctx mvd_ctx;   /* opaque; created by mvd_create, freed by mvd_destroy */
+
+typedef enum {
+  MVD_OK = 0,
+  MVD_ERR_INVALID_ARG = 1,   /* NULL pointer, bad dims, even PSF size, PSF larger than volume, bad enum */
+  MVD_ERR_UNSUPPORTED = 2,   /* no FFT length available for this size */
+  MVD_ERR_WORKSPACE = 3,     /* workspace NULL, misaligned or too small */
+  MVD_ERR_CUDA = 4,          /* a CUDA call failed (see mvd_last_error) */
+  MVD_ERR_STATE = 5          /* context unusable after an earlier CUDA error */
+} mvd_status;
+
+typedef enum {
+  MVD_INDEPENDENT = 0,       /* eq. 70:  combined update, back-projector P_v*              */
+  MVD_EFFICIENT = 1,         /* eq. 104: combined update, back-projector P_v^compound      */
+  MVD_OSEM = 2               /* eq. 109-112: sequential updates, back-projector per kernel_mode */
+} mvd_variant;
+
+typedef enum {
+  MVD_KERNEL_AUTO = 0,       /* INDEPENDENT -> PLAIN; EFFICIENT, OSEM -> COMPOUND (R2)     */
+  MVD_KERNEL_PLAIN = 1,      /* with MVD_OSEM: classical OS-EM, eq. 114-117       */
+  MVD_KERNEL_COMPOUND = 2,
+  MVD_KERNEL_OPT1 = 3,
+  MVD_KERNEL_OPT2 = 4
+} mvd_kernel_mode;
+
+typedef struct {
+  size_t struct_size;        /* = sizeof(mvd_options); lets the struct grow compatibly      */
+  int kernel_mode;           /* mvd_kernel_mode                                             */
+  int literal_product;       /* combined variants: 0 = |V|-th root (eq. 44, default), 1 = bare product of eq. 2/38/104 */
+  float eps;                 /* denominator clamp, <= 0 -> default 1e-6 (R4)                */
+  float psi_floor;           /* estimate floor,    <  0 -> default 1e-6 (R4); 0 allowed     */
+  const float* psi0;         /* optional DEVICE pointer to an initial estimate (N voxels); NULL -> mean of all views (L304, L421) */
+  int fft_dims[3];           /* {Mx2, My, Mz}; 0 -> the library picks.  Mx2 is the length of the half-row transform */
+  void* workspace;           /* DEVICE pointer, caller owned                                */
+  size_t workspace_bytes;
+  void* stream;              /* cudaStream_t                                                */
+  int use_graph;             /* 1: mvd_iterate replays one captured CUDA graph per iteration */
+} mvd_options;
+
+/* Fills *opt with the defaults (struct_size set, everything else 0/NULL/defaults). */
+MVD_API void mvd_options_init(mvd_options* opt);
+
+/* Bytes of workspace mvd_create needs for this problem; 0 if the arguments are invalid or
+ * unsupported.  `opt` may be NULL (defaults); only kernel_mode and fft_dims are read. */
+MVD_API size_t mvd_workspace_size(int n_views, const int dims[3], const int (*psf_dims)[3],
+                          mvd_variant variant, const mvd_options* opt);
+
+/* The FFT lengths {Mx2, My, Mz} the library would use (for reporting algorithmic bytes). */
+MVD_API mvd_status mvd_plan_dims(int n_views, const int dims[3], const int (*psf_dims)[3],
+                         const mvd_options* opt, int fft_dims_out[3]);
+
+/* Builds a context: normalises the PSFs, computes the back-projectors K_v on the device (eq. 105 /
+ * 107 / 108), their spectra and those of P_v, and the initial estimate.  Synchronises the stream
+ * before returning.  See the header comment for pointer kinds and ownership. */
+MVD_API mvd_status mvd_create(mvd_ctx** out, int n_views,
+                      const float* const* views,      /* n_views DEVICE pointers   */
+                      const int dims[3],
+                      const float* const* psfs,       /* n_views HOST pointers     */
+                      const int (*psf_dims)[3],
+                      mvd_variant variant, const mvd_options* opt /* workspace required */);
+
+/* Advances n >= 0 iterations (asynchronous on the stream). */
+MVD_API mvd_status mvd_iterate(mvd_ctx* ctx, int n);
+
+/* Copies the current estimate (Nx*Ny*Nz floats) to dst: a device pointer if dst_is_device != 0
+ * (asynchronous on the stream), else a host pointer (the stream is synchronised). */
+MVD_API mvd_status mvd_get_estimate(mvd_ctx* ctx, float* dst, int dst_is_device);
+
+/* Replaces the estimate (device pointer, N voxels); resume / fixed-point tests. */
+MVD_API mvd_status mvd_set_estimate(mvd_ctx* ctx, const float* src_device);
+
+/* Statistics of the LAST psi update: flux = sum psi_new, l1_change = sum |psi_new - psi_old|
+ * (the reductions the paper's quality curves use, L127).  Synchronises.  Any pointer may be NULL. */
+MVD_API mvd_status mvd_get_stats(mvd_ctx* ctx, double* flux, double* l1_change, int* iterations_done);
+
+/* Copies back-projector K_v (psf_dims[v] floats... as doubles, x fastest) to a HOST buffer.
+ * Lets tests compare the device precompute (eq. 105) with the oracle directly.  Synchronises. */
+MVD_API mvd_status mvd_get_back_projector(mvd_ctx* ctx, int view, double* dst_host);
+
+/* One zero-extended "same" convolution of a device volume with view v's PSF (which = 0) or
+ * back-projector (which = 1) through the library's FFT path: dst = crop(src (*) kernel).
+ * src and dst are DEVICE pointers to N voxels (may alias).  Uses the context's work buffers: the
+ * next mvd_iterate re-derives its transform state.  For per-stage parity tests. */
+MVD_API mvd_status mvd_convolve(mvd_ctx* ctx, int view, int which, const float* src, float* dst);
+
+/* Number of kernel launches the library has issued on this context since creation. */
+MVD_API long long mvd_launch_count(const mvd_ctx* ctx);
+
+/* Block-wise processing (L64, L943; R13): tiles the volume into blocks of block_dims, extends
+ * every block by `halo` voxels of neighbouring data per side (clipped at the volume faces; halo
+ * = NULL -> PSF half-size), runs `iterations` iterations on each extended block with
+ * psi0 = mean over the whole volume, and pastes the central block into dst (DEVICE, N voxels).
+ * All device memory comes from opt->workspace (size: mvd_blocked_workspace_size). */
+MVD_API size_t mvd_blocked_workspace_size(int n_views, const int dims[3], const int (*psf_dims)[3],
+                                  mvd_variant variant, const mvd_options* opt,
+                                  const int block_dims[3], const int halo[3]);
+MVD_API mvd_status mvd_deconvolve_blocked(int n_views, const float* const* views, const int dims[3],
+                                  const float* const* psfs, const int (*psf_dims)[3],
+                                  mvd_variant variant, const mvd_options* opt,
+                                  const int block_dims[3], const int halo[3], int iterations,
+                                  float* dst_device, long long* launches_out);
+
+MVD_API void mvd_destroy(mvd_ctx* ctx);                    /* NULL-safe */
+MVD_API const char* mvd_status_string(mvd_status s);
+MVD_API const char* mvd_last_error(const mvd_ctx* ctx);    /* "" if none; valid until the next call */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MVD_H_ */

@@ -1,0 +1,317 @@
+"""Thin Python binding of libmvd.so (include/mvd.h): argument marshalling only.
+
+Every step of the deconvolution runs in the library's CUDA kernels; PyTorch is used here only to
+own device memory (views, workspace, results) and to supply the stream.  There is no CPU path: if
+libmvd.so is missing or no CUDA device is present, constructing a Deconvolver raises.
+The function names mirror the C ABI (mvd_create / mvd_iterate / mvd_get_estimate ...).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmvd.so")
+
+VARIANTS = {"independent": 0, "efficient": 1, "osem": 2}
+KERNEL_MODES = {"auto": 0, "plain": 1, "compound": 2, "opt1": 3, "opt2": 4}
+
+# every symbol include/mvd.h declares (tests check that the library exports them all)
+SYMBOLS = (
+    "mvd_options_init", "mvd_workspace_size", "mvd_plan_dims", "mvd_create", "mvd_iterate",
+    "mvd_get_estimate", "mvd_set_estimate", "mvd_get_stats", "mvd_get_back_projector", "mvd_convolve",
+    "mvd_launch_count", "mvd_blocked_workspace_size", "mvd_deconvolve_blocked", "mvd_destroy",
+    "mvd_status_string", "mvd_last_error",
+)
+
+
+class MvdError(RuntimeError):
+    pass
+
+
+class mvd_options(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_size_t),
+        ("kernel_mode", C.c_int),
+        ("literal_product", C.c_int),
+        ("eps", C.c_float),
+        ("psi_floor", C.c_float),
+        ("psi0", C.c_void_p),
+        ("fft_dims", C.c_int * 3),
+        ("workspace", C.c_void_p),
+        ("workspace_bytes", C.c_size_t),
+        ("stream", C.c_void_p),
+        ("use_graph", C.c_int),
+    ]
+
+
+_Int3 = C.c_int * 3
+_lib = None
+
+
+def load_library():
+    """dlopen libmvd.so (built in-tree by ``python -m paper_1308_0730_b200.build``)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise MvdError("%s not found: build it with `python -m paper_1308_0730_b200.build` "
+                       "(there is no CPU fallback)" % LIB_PATH)
+    lib = C.CDLL(LIB_PATH)
+    vp, ip = C.c_void_p, C.POINTER(C.c_int)
+    lib.mvd_options_init.argtypes = [C.POINTER(mvd_options)]
+    lib.mvd_options_init.restype = None
+    lib.mvd_workspace_size.argtypes = [C.c_int, _Int3, vp, C.c_int, C.POINTER(mvd_options)]
+    lib.mvd_workspace_size.restype = C.c_size_t
+    lib.mvd_plan_dims.argtypes = [C.c_int, _Int3, vp, C.POINTER(mvd_options), _Int3]
+    lib.mvd_plan_dims.restype = C.c_int
+    lib.mvd_create.argtypes = [C.POINTER(vp), C.c_int, C.POINTER(vp), _Int3, C.POINTER(vp), vp, C.c_int,
+                               C.POINTER(mvd_options)]
+    lib.mvd_create.restype = C.c_int
+    lib.mvd_iterate.argtypes = [vp, C.c_int]
+    lib.mvd_iterate.restype = C.c_int
+    lib.mvd_get_estimate.argtypes = [vp, vp, C.c_int]
+    lib.mvd_get_estimate.restype = C.c_int
+    lib.mvd_set_estimate.argtypes = [vp, vp]
+    lib.mvd_set_estimate.restype = C.c_int
+    lib.mvd_get_stats.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), ip]
+    lib.mvd_get_stats.restype = C.c_int
+    lib.mvd_get_back_projector.argtypes = [vp, C.c_int, vp]
+    lib.mvd_get_back_projector.restype = C.c_int
+    lib.mvd_convolve.argtypes = [vp, C.c_int, C.c_int, vp, vp]
+    lib.mvd_convolve.restype = C.c_int
+    lib.mvd_launch_count.argtypes = [vp]
+    lib.mvd_launch_count.restype = C.c_longlong
+    lib.mvd_blocked_workspace_size.argtypes = [C.c_int, _Int3, vp, C.c_int, C.POINTER(mvd_options), _Int3, vp]
+    lib.mvd_blocked_workspace_size.restype = C.c_size_t
+    lib.mvd_deconvolve_blocked.argtypes = [C.c_int, C.POINTER(vp), _Int3, C.POINTER(vp), vp, C.c_int,
+                                           C.POINTER(mvd_options), _Int3, vp, C.c_int, vp,
+                                           C.POINTER(C.c_longlong)]
+    lib.mvd_deconvolve_blocked.restype = C.c_int
+    lib.mvd_destroy.argtypes = [vp]
+    lib.mvd_destroy.restype = None
+    lib.mvd_status_string.argtypes = [C.c_int]
+    lib.mvd_status_string.restype = C.c_char_p
+    lib.mvd_last_error.argtypes = [vp]
+    lib.mvd_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(status, ctx=None, what=""):
+    if status != 0:
+        lib = load_library()
+        msg = lib.mvd_status_string(status).decode()
+        detail = lib.mvd_last_error(ctx).decode() if ctx else ""
+        raise MvdError("%s: %s%s" % (what, msg, (" (" + detail + ")") if detail else ""))
+
+
+def _psf_args(psfs):
+    """Host PSF arrays (Kz,Ky,Kx) -> (keepalive arrays, void* array, int[V][3] of {Kx,Ky,Kz})."""
+    arrs = [np.ascontiguousarray(p, dtype=np.float32) for p in psfs]
+    for a in arrs:
+        if a.ndim != 3:
+            raise MvdError("a PSF must be a 3-D array (Kz, Ky, Kx)")
+    ptrs = (C.c_void_p * len(arrs))(*[a.ctypes.data for a in arrs])
+    dims = (C.c_int * (3 * len(arrs)))()
+    for v, a in enumerate(arrs):
+        dims[3 * v + 0], dims[3 * v + 1], dims[3 * v + 2] = a.shape[2], a.shape[1], a.shape[0]
+    return arrs, ptrs, dims
+
+
+def _make_options(kernel_mode, literal_product, eps, psi_floor, fft_dims, use_graph):
+    lib = load_library()
+    opt = mvd_options()
+    lib.mvd_options_init(C.byref(opt))
+    opt.kernel_mode = KERNEL_MODES[kernel_mode]
+    opt.literal_product = int(bool(literal_product))
+    if eps is not None:
+        opt.eps = float(eps)
+    if psi_floor is not None:
+        opt.psi_floor = float(psi_floor)
+    if fft_dims is not None:
+        opt.fft_dims[:] = [int(x) for x in fft_dims]
+    opt.use_graph = int(bool(use_graph))
+    return opt
+
+
+def plan_dims(dims, psfs_or_dims, kernel_mode="auto", fft_dims=None):
+    """FFT lengths (Mx2, My, Mz) the library uses for volume dims (Nx,Ny,Nz) and PSF boxes
+    [(Kx,Ky,Kz), ...].  Pure host logic: works without a GPU."""
+    lib = load_library()
+    boxes = [tuple(int(x) for x in b) for b in psfs_or_dims]
+    pd = (C.c_int * (3 * len(boxes)))(*[x for b in boxes for x in b])
+    opt = _make_options(kernel_mode, False, None, None, fft_dims, False)
+    out = _Int3()
+    _check(lib.mvd_plan_dims(len(boxes), _Int3(*dims), C.cast(pd, C.c_void_p), C.byref(opt), out), None, "mvd_plan_dims")
+    return tuple(out)
+
+
+def workspace_size(dims, boxes, variant="osem", kernel_mode="auto", fft_dims=None):
+    lib = load_library()
+    pd = (C.c_int * (3 * len(boxes)))(*[int(x) for b in boxes for x in b])
+    opt = _make_options(kernel_mode, False, None, None, fft_dims, False)
+    return int(lib.mvd_workspace_size(len(boxes), _Int3(*dims), C.cast(pd, C.c_void_p), VARIANTS[variant], C.byref(opt)))
+
+
+class Deconvolver:
+    """One mvd_ctx.  ``views``: list of CUDA float32 torch tensors of shape (Nz,Ny,Nx) (borrowed, kept
+    alive here); ``psfs``: list of host arrays (Kz,Ky,Kx)."""
+
+    def __init__(self, views, psfs, variant="osem", kernel_mode="auto", literal_product=False,
+                 eps=None, psi_floor=None, psi0=None, fft_dims=None, use_graph=False, stream=None):
+        import torch
+
+        lib = load_library()
+        if not torch.cuda.is_available():
+            raise MvdError("no CUDA device: the multi-view deconvolution path has no CPU fallback")
+        if len(views) != len(psfs) or not views:
+            raise MvdError("need one PSF per view")
+        self._torch = torch
+        self.views = [v if (v.is_cuda and v.dtype == torch.float32 and v.is_contiguous())
+                      else v.to(device="cuda", dtype=torch.float32).contiguous() for v in views]
+        shape = tuple(self.views[0].shape)
+        if len(shape) != 3 or any(tuple(v.shape) != shape for v in self.views):
+            raise MvdError("views must be 3-D tensors of one shape (Nz, Ny, Nx)")
+        self.shape = shape
+        self.dims = (shape[2], shape[1], shape[0])
+        self.device = self.views[0].device
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._psfs, psf_ptrs, psf_dims = _psf_args(psfs)
+        self._psf_dims = psf_dims
+        opt = _make_options(kernel_mode, literal_product, eps, psi_floor, fft_dims, use_graph)
+        nbytes = lib.mvd_workspace_size(len(views), _Int3(*self.dims), C.cast(psf_dims, C.c_void_p),
+                                        VARIANTS[variant], C.byref(opt))
+        if nbytes == 0:
+            raise MvdError("mvd_workspace_size: invalid or unsupported problem "
+                           "(dims %s, PSF boxes %s)" % (self.dims, [tuple(p.shape[::-1]) for p in self._psfs]))
+        with torch.cuda.stream(self.stream):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) // 256 * 256
+        opt.workspace = base
+        opt.workspace_bytes = nbytes
+        opt.stream = self.stream.cuda_stream
+        self._psi0 = None
+        if psi0 is not None:
+            self._psi0 = psi0.to(device=self.device, dtype=torch.float32).contiguous()
+            opt.psi0 = self._psi0.data_ptr()
+        self.workspace_bytes = int(nbytes)
+        view_ptrs = (C.c_void_p * len(views))(*[v.data_ptr() for v in self.views])
+        ctx = C.c_void_p()
+        with torch.cuda.device(self.device):
+            st = lib.mvd_create(C.byref(ctx), len(views), view_ptrs, _Int3(*self.dims), psf_ptrs,
+                                C.cast(psf_dims, C.c_void_p), VARIANTS[variant], C.byref(opt))
+        _check(st, None, "mvd_create")
+        self._ctx = ctx
+        self._lib = lib
+        out = _Int3()
+        lib.mvd_plan_dims(len(views), _Int3(*self.dims), C.cast(psf_dims, C.c_void_p), C.byref(opt), out)
+        self.fft_dims = tuple(out)
+
+    # -- C ABI mirrors --------------------------------------------------------------------------
+    def iterate(self, n=1):
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.mvd_iterate(self._ctx, int(n)), self._ctx, "mvd_iterate")
+
+    def get_estimate(self, out=None):
+        """Device tensor (Nz,Ny,Nx) with a copy of psi (asynchronous on the stream)."""
+        torch = self._torch
+        if out is None:
+            with torch.cuda.stream(self.stream):
+                out = torch.empty(self.shape, dtype=torch.float32, device=self.device)
+        _check(self._lib.mvd_get_estimate(self._ctx, out.data_ptr(), 1), self._ctx, "mvd_get_estimate")
+        return out
+
+    def get_estimate_host(self, out=None):
+        """numpy array (Nz,Ny,Nx); synchronises.  ``out`` may be a (pinned) float32 array."""
+        if out is None:
+            out = np.empty(self.shape, dtype=np.float32)
+        _check(self._lib.mvd_get_estimate(self._ctx, out.ctypes.data, 0), self._ctx, "mvd_get_estimate")
+        return out
+
+    def set_estimate(self, psi):
+        t = psi.to(device=self.device, dtype=self._torch.float32).contiguous()
+        if tuple(t.shape) != self.shape:
+            raise MvdError("estimate has the wrong shape")
+        self.stream.wait_stream(self._torch.cuda.current_stream(self.device))
+        _check(self._lib.mvd_set_estimate(self._ctx, t.data_ptr()), self._ctx, "mvd_set_estimate")
+        self.stream.synchronize()
+
+    def get_stats(self):
+        f, l, it = C.c_double(), C.c_double(), C.c_int()
+        _check(self._lib.mvd_get_stats(self._ctx, C.byref(f), C.byref(l), C.byref(it)), self._ctx, "mvd_get_stats")
+        return {"flux": f.value, "l1_change": l.value, "iterations_done": it.value}
+
+    def get_back_projector(self, view):
+        p = self._psfs[view]
+        out = np.empty(p.shape, dtype=np.float64)
+        _check(self._lib.mvd_get_back_projector(self._ctx, int(view), out.ctypes.data), self._ctx, "mvd_get_back_projector")
+        return out
+
+    def convolve(self, view, which, src):
+        """crop(src (*) P_view) (which=0) or crop(src (*) K_view) (which=1) through the FFT path."""
+        torch = self._torch
+        s = src.to(device=self.device, dtype=torch.float32).contiguous()
+        self.stream.wait_stream(torch.cuda.current_stream(self.device))
+        with torch.cuda.stream(self.stream):
+            dst = torch.empty(self.shape, dtype=torch.float32, device=self.device)
+        _check(self._lib.mvd_convolve(self._ctx, int(view), int(which), s.data_ptr(), dst.data_ptr()), self._ctx, "mvd_convolve")
+        self.stream.synchronize()
+        return dst
+
+    @property
+    def launch_count(self):
+        return int(self._lib.mvd_launch_count(self._ctx))
+
+    def close(self):
+        if getattr(self, "_ctx", None):
+            self.stream.synchronize()
+            self._lib.mvd_destroy(self._ctx)
+            self._ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def deconvolve_blocked(views, psfs, block_dims, iterations, variant="osem", kernel_mode="auto",
+                       halo=None, eps=None, psi_floor=None, literal_product=False, stream=None):
+    """mvd_deconvolve_blocked: block_dims / halo are (x,y,z).  Returns (device tensor, launches)."""
+    import torch
+
+    lib = load_library()
+    if not torch.cuda.is_available():
+        raise MvdError("no CUDA device: the multi-view deconvolution path has no CPU fallback")
+    views = [v.to(device="cuda", dtype=torch.float32).contiguous() for v in views]
+    shape = tuple(views[0].shape)
+    dims = (shape[2], shape[1], shape[0])
+    device = views[0].device
+    stream = stream if stream is not None else torch.cuda.current_stream(device)
+    keep, psf_ptrs, psf_dims = _psf_args(psfs)
+    opt = _make_options(kernel_mode, literal_product, eps, psi_floor, None, False)
+    halo_arg = C.cast(_Int3(*halo), C.c_void_p) if halo is not None else None
+    nbytes = lib.mvd_blocked_workspace_size(len(views), _Int3(*dims), C.cast(psf_dims, C.c_void_p),
+                                            VARIANTS[variant], C.byref(opt), _Int3(*block_dims), halo_arg)
+    if nbytes == 0:
+        raise MvdError("mvd_blocked_workspace_size: invalid or unsupported problem")
+    with torch.cuda.stream(stream):
+        ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
+        dst = torch.empty(shape, dtype=torch.float32, device=device)
+    opt.workspace = (ws.data_ptr() + 255) // 256 * 256
+    opt.workspace_bytes = nbytes
+    opt.stream = stream.cuda_stream
+    view_ptrs = (C.c_void_p * len(views))(*[v.data_ptr() for v in views])
+    launches = C.c_longlong(0)
+    with torch.cuda.device(device):
+        st = lib.mvd_deconvolve_blocked(len(views), view_ptrs, _Int3(*dims), psf_ptrs,
+                                        C.cast(psf_dims, C.c_void_p), VARIANTS[variant], C.byref(opt),
+                                        _Int3(*block_dims), halo_arg, int(iterations), dst.data_ptr(),
+                                        C.byref(launches))
+    _check(st, None, "mvd_deconvolve_blocked")
+    stream.synchronize()
+    del keep
+    return dst, int(launches.value)

@@ -1,0 +1,84 @@
+// Host-visible description of the per-length transform kernels (one LengthOps per supported
+// pencil length M = A*B).  The kernels themselves are templates in pass_kernels.cuh and are
+// instantiated once per length in inst.cu; mvd.cu only sees this table.
+#pragma once
+
+#include <cuda_runtime.h>
+
+namespace mvd {
+
+// ---- strided pencil FFT (y pass, plain z pass): pencils along a strided axis, tiles of T
+//      contiguous complex elements across the unit-stride axis --------------------------------
+struct StridedArgs {
+  const float2* in;
+  float2* out;
+  const float2* tw;        // tw[j] = exp(-2*pi*i*j/M), j < M
+  int T;                   // tile width (contiguous complex elements)
+  int nthreads;
+  int tiles_per_line;
+  long long line_len;      // contiguous extent
+  long long n_outer;       // number of lines
+  long long in_outer_stride, out_outer_stride;
+  long long in_pstride, out_pstride;   // element stride along the pencil
+  int n_in;                // pencil inputs >= n_in are zero (never read)
+  int n_out;               // pencil outputs >= n_out are not stored
+};
+
+// ---- fused z pass: forward FFT along z, multiply by a kernel spectrum, inverse FFT ----------
+struct ZconvArgs {
+  const float2* in;
+  float2* out;
+  const float2* spec;      // [Mz][plane] complex, already scaled by 1/(Mx*My*Mz)
+  const float2* tw;
+  int T;
+  int nthreads;
+  long long plane;         // My*Mx2: element stride along z, and the contiguous extent
+  int nz;                  // planes read and written (zero padding beyond is implicit)
+};
+
+// ---- fused row pass along x (see pass_kernels.cuh for the half-row packing) -------------------
+enum XMode {
+  X_LOAD = 0,              // (psi | complex rows) -> forward FFT
+  X_QUOT = 1,              // inverse FFT -> q = phi / max(b, eps) -> forward FFT
+  X_UPDATE = 2,            // inverse FFT -> psi <- max(psi*f, floor) -> forward FFT   (OSEM)
+  X_ACCUM = 3              // inverse FFT -> raw store | product accumulation | final combined update
+};
+enum AccMode { ACC_STORE = 0, ACC_FIRST = 1, ACC_MID = 2, ACC_LAST = 3, ACC_ONLY = 4 };
+
+struct XArgs {
+  const float2* in;        // work buffer rows (inverse input)
+  float2* out;             // work buffer rows (forward output)
+  const float2* tw;
+  int rows_per_cta;
+  int nthreads;
+  long long nrows;         // rows processed = ny_rows * nz
+  int ny_rows;             // rows used per plane
+  long long plane_pitch;   // elements between planes of the work buffer (My*Mx2)
+  int nx;                  // real row length Nx
+  int hx;                  // (Nx+1)/2: element n of the half row carries x=n (re) and x=n+hx (im)
+  int rx;                  // PSF half-size along x of this view
+  const float* phi;        // X_QUOT: view; X_LOAD: psi (real input)
+  float* psi;              // X_UPDATE / ACC_LAST: estimate, updated in place
+  float* acc;              // X_ACCUM: product accumulator / raw destination
+  double* partials;        // per-CTA {flux, l1} (X_UPDATE, ACC_LAST)
+  float eps, psi_floor, inv_nviews;
+  int acc_mode;            // AccMode
+  int literal_product;
+  int complex_in;          // X_LOAD: rows of `in` are complex and transformed in full
+};
+
+struct LengthOps {
+  int M, A, B;
+  int max_threads;         // launch bound of the kernels of this length
+  cudaError_t (*init)();   // opt in to > 48 KB dynamic shared memory
+  cudaError_t (*strided)(const StridedArgs&, int dir, cudaStream_t);
+  cudaError_t (*zconv)(const ZconvArgs&, cudaStream_t);
+  cudaError_t (*xrow)(const XArgs&, int mode, cudaStream_t);
+  size_t (*strided_smem)(int T);
+  size_t (*xrow_smem)(int rows, int rx);
+};
+
+// table of all compiled lengths, ascending in M
+const LengthOps* const* length_table(int* count);
+
+}  // namespace mvd

@@ -1,0 +1,191 @@
+// Kernels that do not depend on the pencil length: reductions (flux, mean, statistics), the
+// back-projector precompute of eq. 105 / 107 / 108 in fp64, the placement of
+// a kernel into its (wrapped, zero-padded) spectrum buffer, and block gather / paste (L943).
+#pragma once
+
+#include <cuda_runtime.h>
+
+namespace mvd {
+
+// ---------------------------------------------------------------------------------------
+// warp-shuffle block reduction of doubles (blockDim.x <= 1024)
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  return v;
+}
+
+__device__ __forceinline__ double block_sum(double v, double* red /* >= 32 doubles of smem */) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  v = warp_sum(v);
+  __syncthreads();                      // red may still be in use by a previous call
+  if (lane == 0) red[warp] = v;
+  __syncthreads();
+  const int nw = (blockDim.x + 31) >> 5;
+  v = (threadIdx.x < nw) ? red[threadIdx.x] : 0.0;
+  if (warp == 0) v = warp_sum(v);
+  return v;                             // valid in thread 0
+}
+
+// partial sums of a float volume: out[blockIdx.x] = sum of this block's grid-stride share
+__global__ void __launch_bounds__(256) sum_f32_kernel(const float* __restrict__ a, long long n,
+                                                      double* __restrict__ partial) {
+  __shared__ double red[32];
+  double s = 0.0;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long n4 = ((reinterpret_cast<size_t>(a) & 15) == 0) ? n / 4 : 0;
+  const float4* a4 = reinterpret_cast<const float4*>(a);
+  for (long long j = i; j < n4; j += stride) {
+    const float4 v = __ldg(a4 + j);
+    s += (double)v.x + (double)v.y + (double)v.z + (double)v.w;
+  }
+  for (long long j = n4 * 4 + i; j < n; j += stride) s += (double)__ldg(a + j);
+  s = block_sum(s, red);
+  if (threadIdx.x == 0) partial[blockIdx.x] = s;
+}
+
+// out[c] = sum_i partial[c + ncol*i], i < n  (single block; ncol <= 2 columns used here)
+__global__ void __launch_bounds__(256) final_sum_kernel(const double* __restrict__ partial, int n,
+                                                        int ncol, double* __restrict__ out) {
+  __shared__ double red[32];
+  for (int c = 0; c < ncol; ++c) {
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) s += partial[(size_t)i * ncol + c];
+    s = block_sum(s, red);
+    if (threadIdx.x == 0) out[c] = s;
+  }
+}
+
+// psi <- (sum_v sums[v]) / count        (psi^0 = average intensity, L304 / L421)
+__global__ void fill_mean_kernel(float* __restrict__ psi, long long n, const double* __restrict__ sums,
+                                 int nsums, double count) {
+  double t = 0.0;
+  for (int v = 0; v < nsums; ++v) t += sums[v];
+  const float m = (float)(t / count);
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) psi[i] = m;
+}
+
+// ---------------------------------------------------------------------------------------
+// PSFs and back-projectors, fp64, x fastest, dims {Kx,Ky,Kz}
+// ---------------------------------------------------------------------------------------
+// dst = src / sum(src)   (eq. 4); src float or double; one block
+template <class Tin>
+__global__ void __launch_bounds__(1024) normalise_kernel(const Tin* __restrict__ src, int n,
+                                                         double* __restrict__ dst) {
+  __shared__ double red[32];
+  __shared__ double total;
+  double s = 0.0;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) s += (double)src[i];
+  s = block_sum(s, red);
+  if (threadIdx.x == 0) total = s;
+  __syncthreads();
+  const double inv = 1.0 / total;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) dst[i] = (double)src[i] * inv;
+}
+
+struct Dims3 { int x, y, z; };
+
+// a[m] = (P (*) flip P)[m] = sum_u P[u] P[u + K-1-m], m in [0, 2K-1) per axis   (P_w (*) P_w*)
+__global__ void __launch_bounds__(128) autocorr_kernel(const double* __restrict__ P, Dims3 K,
+                                                       double* __restrict__ a) {
+  const Dims3 G{2 * K.x - 1, 2 * K.y - 1, 2 * K.z - 1};
+  const long long tot = (long long)G.x * G.y * G.z;
+  const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= tot) return;
+  const int mx = int(m % G.x), my = int((m / G.x) % G.y), mz = int(m / ((long long)G.x * G.y));
+  const int sx = K.x - 1 - mx, sy = K.y - 1 - my, sz = K.z - 1 - mz;   // u' = u + s
+  double acc = 0.0;
+  for (int uz = max(0, -sz); uz < min(K.z, K.z - sz); ++uz)
+    for (int uy = max(0, -sy); uy < min(K.y, K.y - sy); ++uy) {
+      const double* p0 = P + ((long long)uz * K.y + uy) * K.x;
+      const double* p1 = P + ((long long)(uz + sz) * K.y + (uy + sy)) * K.x + sx;
+      for (int ux = max(0, -sx); ux < min(K.x, K.x - sx); ++ux) acc += p0[ux] * p1[ux];
+    }
+  a[m] = acc;
+}
+
+// kern[j] *= sum_u flipPv[u] G[off + j - u],  flipPv[u] = Pv[K-1-u], off = (Gd-1)/2, j in the box of
+// P_v: the central crop of the full convolution P_v* (*) G (R6).  G = P_w (*) P_w* (eq. 105) or P_w (eq. 107).
+__global__ void __launch_bounds__(128) corr_crop_mul_kernel(const double* __restrict__ Pv, Dims3 K,
+                                                            const double* __restrict__ G, Dims3 Gd,
+                                                            double* __restrict__ kern) {
+  const long long tot = (long long)K.x * K.y * K.z;
+  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= tot) return;
+  const int jx = int(j % K.x), jy = int((j / K.x) % K.y), jz = int(j / ((long long)K.x * K.y));
+  const int ox = (Gd.x - 1) / 2 + jx, oy = (Gd.y - 1) / 2 + jy, oz = (Gd.z - 1) / 2 + jz;
+  double acc = 0.0;
+  // g index = o - u in [0, Gd)  ->  u in (o - Gd, o]
+  for (int uz = max(0, oz - Gd.z + 1); uz <= min(K.z - 1, oz); ++uz)
+    for (int uy = max(0, oy - Gd.y + 1); uy <= min(K.y - 1, oy); ++uy) {
+      const double* pv = Pv + ((long long)(K.z - 1 - uz) * K.y + (K.y - 1 - uy)) * K.x;
+      const double* g = G + ((long long)(oz - uz) * Gd.y + (oy - uy)) * Gd.x;
+      for (int ux = max(0, ox - Gd.x + 1); ux <= min(K.x - 1, ox); ++ux)
+        acc += pv[K.x - 1 - ux] * g[ox - ux];
+    }
+  kern[j] *= acc;
+}
+
+// kern[j] = (P[K-1-j])^power  (mirror, L312; power = V gives eq. 108, R9)
+__global__ void flip_pow_kernel(const double* __restrict__ P, Dims3 K, int power,
+                                double* __restrict__ kern) {
+  const long long tot = (long long)K.x * K.y * K.z;
+  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= tot) return;
+  const double v = P[tot - 1 - j];     // mirroring all three axes = reversing the flat index
+  double r = v;
+  for (int i = 1; i < power; ++i) r *= v;
+  kern[j] = r;
+}
+
+// spectrum buffer <- kernel taps at their wrapped positions: tap u (centre c = (K-1)/2) goes to
+// ((u - c) mod M) per axis; value scaled (1/(Mx*My*Mz) folds the inverse-FFT normalisation in)
+__global__ void scatter_kernel(const double* __restrict__ kern, Dims3 K, float2* __restrict__ spec,
+                               Dims3 M, double scale) {
+  const long long tot = (long long)K.x * K.y * K.z;
+  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= tot) return;
+  const int jx = int(j % K.x), jy = int((j / K.x) % K.y), jz = int(j / ((long long)K.x * K.y));
+  int wx = jx - (K.x - 1) / 2, wy = jy - (K.y - 1) / 2, wz = jz - (K.z - 1) / 2;
+  if (wx < 0) wx += M.x;
+  if (wy < 0) wy += M.y;
+  if (wz < 0) wz += M.z;
+  spec[((long long)wz * M.y + wy) * M.x + wx] = make_float2((float)(kern[j] * scale), 0.f);
+}
+
+// ---------------------------------------------------------------------------------------
+// block-wise processing (L64, L943; R13)
+// ---------------------------------------------------------------------------------------
+// dst (dims E) <- src (dims N) [o .. o+E)
+__global__ void gather_block_kernel(const float* __restrict__ src, Dims3 N, Dims3 o, Dims3 E,
+                                    float* __restrict__ dst) {
+  const long long tot = (long long)E.x * E.y * E.z;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < tot; i += stride) {
+    const int x = int(i % E.x), y = int((i / E.x) % E.y), z = int(i / ((long long)E.x * E.y));
+    dst[i] = src[((long long)(z + o.z) * N.y + (y + o.y)) * N.x + (x + o.x)];
+  }
+}
+
+// dst (dims N) [d .. d+C) <- src (dims E) [s .. s+C)
+__global__ void paste_block_kernel(const float* __restrict__ src, Dims3 E, Dims3 s, Dims3 C,
+                                   float* __restrict__ dst, Dims3 N, Dims3 d) {
+  const long long tot = (long long)C.x * C.y * C.z;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < tot; i += stride) {
+    const int x = int(i % C.x), y = int((i / C.x) % C.y), z = int(i / ((long long)C.x * C.y));
+    dst[((long long)(z + d.z) * N.y + (y + d.y)) * N.x + (x + d.x)] =
+        src[((long long)(z + s.z) * E.y + (y + s.y)) * E.x + (x + s.x)];
+  }
+}
+
+__global__ void fill_const_kernel(float* __restrict__ a, long long n, const float* __restrict__ value) {
+  const float m = *value;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) a[i] = m;
+}
+
+}  // namespace mvd

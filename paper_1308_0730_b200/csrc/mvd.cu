@@ -1,0 +1,884 @@
+// libmvd.so: context, planner and launch sequences behind the C ABI of include/mvd.h.
+//
+// Path per view-update (eq. 1, eq. 13, eq. 104,
+// eq. 109-112), all on the device, one stream:
+//   y-forward -> [z-forward . P_v spectrum . z-inverse] -> y-inverse
+//     -> [x-inverse -> quotient phi_v/max(b,eps) -> x-forward]
+//   y-forward -> [z-forward . K_v spectrum . z-inverse] -> y-inverse
+//     -> [x-inverse -> psi update (or product accumulation) -> x-forward of the new psi]
+// The oracle (oracle/) is never used here; without a CUDA device every call fails with
+// MVD_ERR_CUDA.
+#include "../../include/mvd.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <array>
+#include <vector>
+
+#include "fft_ops.h"
+#include "misc_kernels.cuh"
+
+namespace mvd {
+
+// ---------------------------------------------------------------------------------------
+// table of compiled lengths (one object file per line of lengths.def)
+// ---------------------------------------------------------------------------------------
+#define MVD_LEN(A, B) extern const LengthOps ops_##A##_##B;
+#include "lengths.def"
+#undef MVD_LEN
+
+static const LengthOps* const g_lengths_unsorted[] = {
+#define MVD_LEN(A, B) &ops_##A##_##B,
+#include "lengths.def"
+#undef MVD_LEN
+};
+
+const LengthOps* const* length_table(int* count) {
+  static std::vector<const LengthOps*> sorted = [] {
+    std::vector<const LengthOps*> v(std::begin(g_lengths_unsorted), std::end(g_lengths_unsorted));
+    std::sort(v.begin(), v.end(), [](const LengthOps* a, const LengthOps* b) { return a->M < b->M; });
+    return v;
+  }();
+  *count = (int)sorted.size();
+  return sorted.data();
+}
+
+static const LengthOps* find_length(int min_len, int exact) {
+  int n;
+  const LengthOps* const* t = length_table(&n);
+  for (int i = 0; i < n; ++i) {
+    if (exact > 0) {
+      if (t[i]->M == exact) return t[i]->M >= min_len ? t[i] : nullptr;
+    } else if (t[i]->M >= min_len) {
+      return t[i];
+    }
+  }
+  return nullptr;
+}
+
+// ---------------------------------------------------------------------------------------
+// plan: sizes, FFT lengths, tiles, workspace layout
+// ---------------------------------------------------------------------------------------
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+static inline int round_up32(int x) { return (x + 31) / 32 * 32; }
+
+struct Plan {
+  int V = 0;
+  int N[3] = {0, 0, 0};
+  std::vector<Dims3> K;          // per view
+  int r[3] = {0, 0, 0};          // max half-size per axis
+  int hx = 0;
+  const LengthOps *lx = nullptr, *ly = nullptr, *lz = nullptr;
+  int Mx = 0, My = 0, Mz = 0;
+  long long nvox = 0, plane = 0, wsize = 0, ssize = 0;   // elements
+  bool combined = false;
+  int kmode = MVD_KERNEL_PLAIN;
+  // tiles
+  int Ty = 0, nty = 0, Tz = 0, ntz = 0, Tzs = 0, ntzs = 0, Tys = 0, ntys = 0, Rx = 0, ntx = 0;
+  int nctax = 0;
+  // workspace offsets (bytes)
+  size_t off_twx = 0, off_twy = 0, off_twz = 0, off_psi = 0, off_acc = 0, off_w = 0, off_w0 = 0,
+         off_spec = 0, off_psf = 0, off_kern = 0, off_auto = 0, off_stage = 0, off_partials = 0,
+         off_scalars = 0, total = 0;
+  size_t psf_stride = 0, auto_stride = 0;   // elements (doubles) per view
+  int sum_blocks = 0;
+};
+
+static int env_int(const char* name, int dflt) {
+  const char* s = getenv(name);
+  return (s && *s) ? atoi(s) : dflt;
+}
+
+// tile width for a strided pass over a contiguous extent L; single_round: T*max(A,B) <= max_threads
+static void choose_tile(const LengthOps* l, long long L, bool single_round, int force, int* T_out,
+                        int* nthreads_out) {
+  const int ab = std::max(l->A, l->B);
+  const size_t smem_cap = 100 * 1024;
+  int best = 0;
+  double best_score = -1.0;
+  const int cand[] = {16, 20, 24, 32, 28, 12, 8, 4};
+  for (int T : cand) {
+    if (l->strided_smem(T) > smem_cap && T > 4) continue;
+    if (single_round && T * ab > l->max_threads) continue;
+    const double eff = double(L) / double(((L + T - 1) / T) * T);
+    const double seg = T >= 16 ? 1.0 : (T >= 8 ? 0.85 : 0.6);   // short segments waste DRAM bursts
+    const double score = eff * seg;
+    if (score > best_score + 1e-9) { best_score = score; best = T; }
+  }
+  if (best == 0) best = std::max(1, std::min(4, l->max_threads / ab));
+  if (force > 0 && (!single_round || force * ab <= l->max_threads)) best = force;
+  const int items = best * ab;
+  const int rounds = (items + l->max_threads - 1) / l->max_threads;
+  *T_out = best;
+  *nthreads_out = std::min(l->max_threads, round_up32((items + rounds - 1) / rounds));
+}
+
+static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (*psf_dims)[3],
+                            mvd_variant variant, const mvd_options* opt) {
+  if (n_views < 1 || n_views > 4096 || !dims || !psf_dims) return MVD_ERR_INVALID_ARG;
+  if ((int)variant < 0 || (int)variant > 2) return MVD_ERR_INVALID_ARG;
+  int kmode = opt ? opt->kernel_mode : MVD_KERNEL_AUTO;
+  if (kmode < 0 || kmode > 4) return MVD_ERR_INVALID_ARG;
+  if (kmode == MVD_KERNEL_AUTO) kmode = (variant == MVD_INDEPENDENT) ? MVD_KERNEL_PLAIN : MVD_KERNEL_COMPOUND;
+  P.kmode = kmode;
+  P.V = n_views;
+  P.combined = variant != MVD_OSEM;
+  for (int a = 0; a < 3; ++a) {
+    if (dims[a] < 1 || dims[a] > (1 << 20)) return MVD_ERR_INVALID_ARG;
+    P.N[a] = dims[a];
+    P.r[a] = 0;
+  }
+  P.K.resize(n_views);
+  for (int v = 0; v < n_views; ++v) {
+    for (int a = 0; a < 3; ++a) {
+      const int k = psf_dims[v][a];
+      if (k < 1 || (k & 1) == 0 || k > dims[a]) return MVD_ERR_INVALID_ARG;
+      P.r[a] = std::max(P.r[a], (k - 1) / 2);
+    }
+    P.K[v] = Dims3{psf_dims[v][0], psf_dims[v][1], psf_dims[v][2]};
+  }
+  P.hx = (P.N[0] + 1) / 2;
+  const int need[3] = {P.hx + 2 * P.r[0], P.N[1] + P.r[1], P.N[2] + P.r[2]};
+  const LengthOps* l[3];
+  for (int a = 0; a < 3; ++a) {
+    const int want = opt ? opt->fft_dims[a] : 0;
+    if (want < 0) return MVD_ERR_INVALID_ARG;
+    l[a] = find_length(need[a], want);
+    if (!l[a]) return want > 0 ? MVD_ERR_INVALID_ARG : MVD_ERR_UNSUPPORTED;
+  }
+  P.lx = l[0]; P.ly = l[1]; P.lz = l[2];
+  P.Mx = l[0]->M; P.My = l[1]->M; P.Mz = l[2]->M;
+  P.nvox = (long long)P.N[0] * P.N[1] * P.N[2];
+  P.plane = (long long)P.My * P.Mx;
+  P.wsize = P.plane * P.N[2];
+  P.ssize = P.plane * P.Mz;
+
+  choose_tile(P.ly, P.Mx, false, env_int("MVD_TY", 0), &P.Ty, &P.nty);
+  choose_tile(P.lz, P.plane, true, env_int("MVD_TZ", 0), &P.Tz, &P.ntz);
+  choose_tile(P.lz, P.plane, false, 0, &P.Tzs, &P.ntzs);
+  choose_tile(P.ly, P.Mx, false, 0, &P.Tys, &P.ntys);
+  {
+    const int ab = std::max(P.lx->A, P.lx->B);
+    int R = std::max(1, env_int("MVD_XTHREADS", 256) / ab);
+    const int force = env_int("MVD_RX", 0);
+    if (force > 0) R = force;
+    R = std::min(R, std::max(1, P.lx->max_threads / ab));
+    while (R > 1 && P.lx->xrow_smem(R, P.r[0]) > 160 * 1024) --R;
+    P.Rx = R;
+    P.ntx = round_up32(R * ab);
+    // spectrum construction runs the same kernel over My*Mz rows
+    const long long rows_max = std::max((long long)P.N[1] * P.N[2], (long long)P.My * P.Mz);
+    P.nctax = (int)((rows_max + R - 1) / R);
+  }
+
+  // workspace layout
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
+  P.off_twx = take((size_t)P.Mx * sizeof(float2));
+  P.off_twy = take((size_t)P.My * sizeof(float2));
+  P.off_twz = take((size_t)P.Mz * sizeof(float2));
+  P.off_psi = take((size_t)P.nvox * sizeof(float));
+  P.off_acc = take((size_t)P.nvox * sizeof(float));
+  P.off_w = take((size_t)P.wsize * sizeof(float2));
+  P.off_w0 = P.combined ? take((size_t)P.wsize * sizeof(float2)) : 0;
+  P.off_spec = take((size_t)P.ssize * sizeof(float2) * 2 * P.V);
+  size_t kmax = 0, amax = 0;
+  for (int v = 0; v < P.V; ++v) {
+    const Dims3 k = P.K[v];
+    kmax = std::max(kmax, (size_t)k.x * k.y * k.z);
+    amax = std::max(amax, (size_t)(2 * k.x - 1) * (2 * k.y - 1) * (2 * k.z - 1));
+  }
+  P.psf_stride = align_up(kmax, 32);
+  P.auto_stride = align_up(amax, 32);
+  P.off_psf = take(P.psf_stride * sizeof(double) * P.V);
+  P.off_kern = take(P.psf_stride * sizeof(double) * P.V);
+  P.off_auto = take(kmode == MVD_KERNEL_COMPOUND ? P.auto_stride * sizeof(double) * P.V : 256);
+  P.off_stage = take(P.psf_stride * sizeof(float));
+  P.sum_blocks = 1184;   // 148 SMs x 8
+  P.off_partials = take(sizeof(double) * 2 * (size_t)std::max(P.nctax, P.sum_blocks));
+  P.off_scalars = take(sizeof(double) * (size_t)(P.V + 8));
+  P.total = o;
+  return MVD_OK;
+}
+
+}  // namespace mvd
+
+using namespace mvd;
+
+// ---------------------------------------------------------------------------------------
+// context
+// ---------------------------------------------------------------------------------------
+struct mvd_ctx {
+  Plan P;
+  mvd_variant variant = MVD_OSEM;
+  int literal = 0;
+  float eps = 1e-6f, psi_floor = 1e-6f;
+  cudaStream_t stream = nullptr;
+  char* ws = nullptr;
+  std::vector<const float*> views;
+  bool w_valid = false;        // the work buffer holds the x-forward transform of the current psi
+  bool broken = false;
+  bool stats_valid = false;
+  int stats_ncta = 0;
+  int iters = 0;
+  long long launches = 0;
+  int use_graph = 0;
+  cudaGraphExec_t graph_exec = nullptr;
+  long long graph_launches = 0;
+  char err[512] = {0};
+
+  float2* twx() { return reinterpret_cast<float2*>(ws + P.off_twx); }
+  float2* twy() { return reinterpret_cast<float2*>(ws + P.off_twy); }
+  float2* twz() { return reinterpret_cast<float2*>(ws + P.off_twz); }
+  float* psi() { return reinterpret_cast<float*>(ws + P.off_psi); }
+  float* acc() { return reinterpret_cast<float*>(ws + P.off_acc); }
+  float2* W() { return reinterpret_cast<float2*>(ws + P.off_w); }
+  float2* W0() { return reinterpret_cast<float2*>(ws + P.off_w0); }
+  float2* specH(int v) { return reinterpret_cast<float2*>(ws + P.off_spec) + (size_t)(2 * v) * P.ssize; }
+  float2* specK(int v) { return reinterpret_cast<float2*>(ws + P.off_spec) + (size_t)(2 * v + 1) * P.ssize; }
+  double* psf(int v) { return reinterpret_cast<double*>(ws + P.off_psf) + (size_t)v * P.psf_stride; }
+  double* kern(int v) { return reinterpret_cast<double*>(ws + P.off_kern) + (size_t)v * P.psf_stride; }
+  double* autoc(int v) { return reinterpret_cast<double*>(ws + P.off_auto) + (size_t)v * P.auto_stride; }
+  float* stage() { return reinterpret_cast<float*>(ws + P.off_stage); }
+  double* partials() { return reinterpret_cast<double*>(ws + P.off_partials); }
+  double* scalars() { return reinterpret_cast<double*>(ws + P.off_scalars); }   // [0..V) view sums, [V],[V+1] stats
+
+  bool fail(cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return false;
+    snprintf(err, sizeof(err), "%s: %s", what, cudaGetErrorString(e));
+    broken = true;
+    return true;
+  }
+};
+
+#define MVD_CK(call, what) \
+  do { if (c->fail((call), what)) return MVD_ERR_CUDA; } while (0)
+
+namespace {
+
+// ---- pass launchers -------------------------------------------------------------------------
+mvd_status y_pass(mvd_ctx* c, float2* buf, int dir, int nz_planes, bool full) {
+  const Plan& P = c->P;
+  StridedArgs a{};
+  a.in = buf; a.out = buf; a.tw = c->twy();
+  a.T = full ? P.Tys : P.Ty;
+  a.nthreads = full ? P.ntys : P.nty;
+  a.line_len = P.Mx;
+  a.tiles_per_line = (P.Mx + a.T - 1) / a.T;
+  a.n_outer = nz_planes;
+  a.in_outer_stride = a.out_outer_stride = P.plane;
+  a.in_pstride = a.out_pstride = P.Mx;
+  if (full) { a.n_in = P.My; a.n_out = P.My; }
+  else if (dir < 0) { a.n_in = P.N[1]; a.n_out = P.My; }
+  else { a.n_in = P.My; a.n_out = P.N[1]; }
+  MVD_CK(P.ly->strided(a, dir, c->stream), "y pass");
+  ++c->launches;
+  return MVD_OK;
+}
+
+mvd_status z_plain_fwd(mvd_ctx* c, float2* buf) {
+  const Plan& P = c->P;
+  StridedArgs a{};
+  a.in = buf; a.out = buf; a.tw = c->twz();
+  a.T = P.Tzs; a.nthreads = P.ntzs;
+  a.line_len = P.plane;
+  a.tiles_per_line = (int)((P.plane + a.T - 1) / a.T);
+  a.n_outer = 1;
+  a.in_outer_stride = a.out_outer_stride = 0;
+  a.in_pstride = a.out_pstride = P.plane;
+  a.n_in = P.Mz; a.n_out = P.Mz;
+  MVD_CK(P.lz->strided(a, -1, c->stream), "z pass");
+  ++c->launches;
+  return MVD_OK;
+}
+
+mvd_status z_conv(mvd_ctx* c, const float2* in, float2* out, const float2* spec) {
+  const Plan& P = c->P;
+  ZconvArgs a{};
+  a.in = in; a.out = out; a.spec = spec; a.tw = c->twz();
+  a.T = P.Tz; a.nthreads = P.ntz; a.plane = P.plane; a.nz = P.N[2];
+  MVD_CK(P.lz->zconv(a, c->stream), "z convolution pass");
+  ++c->launches;
+  return MVD_OK;
+}
+
+XArgs x_args(mvd_ctx* c, const float2* in, float2* out, int rx) {
+  const Plan& P = c->P;
+  XArgs a{};
+  a.in = in; a.out = out; a.tw = c->twx();
+  a.rows_per_cta = P.Rx; a.nthreads = P.ntx;
+  a.nrows = (long long)P.N[1] * P.N[2];
+  a.ny_rows = P.N[1];
+  a.plane_pitch = P.plane;
+  a.nx = P.N[0]; a.hx = P.hx; a.rx = rx;
+  a.psi = c->psi(); a.acc = c->acc(); a.partials = c->partials();
+  a.eps = c->eps; a.psi_floor = c->psi_floor; a.inv_nviews = 1.0f / (float)P.V;
+  a.literal_product = c->literal;
+  return a;
+}
+
+mvd_status x_pass(mvd_ctx* c, const XArgs& a, int mode) {
+  MVD_CK(c->P.lx->xrow(a, mode, c->stream), "x pass");
+  ++c->launches;
+  if (mode == X_UPDATE || (mode == X_ACCUM && (a.acc_mode == ACC_LAST || a.acc_mode == ACC_ONLY))) {
+    c->stats_valid = true;
+    c->stats_ncta = (int)((a.nrows + a.rows_per_cta - 1) / a.rows_per_cta);
+  }
+  return MVD_OK;
+}
+
+mvd_status x_load(mvd_ctx* c, const float* src, float2* out) {
+  XArgs a = x_args(c, nullptr, out, 0);
+  a.phi = src;
+  return x_pass(c, a, X_LOAD);
+}
+
+#define MVD_TRY(expr) do { mvd_status s_ = (expr); if (s_ != MVD_OK) return s_; } while (0)
+
+// crop(src (*) kernel) with the forward transform of src already in `buf` rows: y, z, y passes
+mvd_status conv_core(mvd_ctx* c, const float2* in, float2* buf, const float2* spec, bool skip_yfwd) {
+  if (!skip_yfwd) MVD_TRY(y_pass(c, buf, -1, c->P.N[2], false));
+  MVD_TRY(z_conv(c, in ? in : buf, buf, spec));
+  MVD_TRY(y_pass(c, buf, +1, c->P.N[2], false));
+  return MVD_OK;
+}
+
+// one iteration (every view contributes once, L817); requires w_valid
+mvd_status iteration_body(mvd_ctx* c) {
+  const Plan& P = c->P;
+  if (!P.combined) {
+    // eq. 109-112: psi updated after every view, index order (R11)
+    for (int v = 0; v < P.V; ++v) {
+      const int rx = (P.K[v].x - 1) / 2;
+      MVD_TRY(conv_core(c, nullptr, c->W(), c->specH(v), false));
+      XArgs q = x_args(c, c->W(), c->W(), rx);
+      q.phi = c->views[v];
+      MVD_TRY(x_pass(c, q, X_QUOT));
+      MVD_TRY(conv_core(c, nullptr, c->W(), c->specK(v), false));
+      XArgs u = x_args(c, c->W(), c->W(), rx);
+      MVD_TRY(x_pass(c, u, X_UPDATE));
+    }
+  } else {
+    // eq. 70 / 104: every f_v from the same psi; the x and y forward passes of psi are shared
+    MVD_TRY(y_pass(c, c->W0(), -1, P.N[2], false));
+    for (int v = 0; v < P.V; ++v) {
+      const int rx = (P.K[v].x - 1) / 2;
+      MVD_TRY(conv_core(c, c->W0(), c->W(), c->specH(v), true));
+      XArgs q = x_args(c, c->W(), c->W(), rx);
+      q.phi = c->views[v];
+      MVD_TRY(x_pass(c, q, X_QUOT));
+      MVD_TRY(conv_core(c, nullptr, c->W(), c->specK(v), false));
+      XArgs u = x_args(c, c->W(), c->W0(), rx);
+      u.acc_mode = P.V == 1 ? ACC_ONLY : (v == 0 ? ACC_FIRST : (v == P.V - 1 ? ACC_LAST : ACC_MID));
+      MVD_TRY(x_pass(c, u, X_ACCUM));
+    }
+  }
+  return MVD_OK;
+}
+
+mvd_status ensure_w(mvd_ctx* c) {
+  if (c->w_valid) return MVD_OK;
+  MVD_TRY(x_load(c, c->psi(), c->P.combined ? c->W0() : c->W()));
+  c->w_valid = true;
+  return MVD_OK;
+}
+
+// ---- precompute (S0) ---------------------------------------------------------------------------
+mvd_status build_spectrum(mvd_ctx* c, const double* kern, Dims3 K, float2* spec) {
+  const Plan& P = c->P;
+  MVD_CK(cudaMemsetAsync(spec, 0, (size_t)P.ssize * sizeof(float2), c->stream), "memset spectrum");
+  const long long tot = (long long)K.x * K.y * K.z;
+  const double scale = 1.0 / ((double)P.Mx * (double)P.My * (double)P.Mz);
+  scatter_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, c->stream>>>(kern, K, spec,
+                                                                        Dims3{P.Mx, P.My, P.Mz}, scale);
+  MVD_CK(cudaGetLastError(), "scatter_kernel");
+  ++c->launches;
+  // x: complex rows, all My*Mz of them, in place
+  XArgs a = x_args(c, spec, spec, 0);
+  a.nrows = (long long)P.My * P.Mz;
+  a.ny_rows = P.My;
+  a.complex_in = 1;
+  MVD_TRY(x_pass(c, a, X_LOAD));
+  // y: every plane of the Mz, full pencils
+  {
+    StridedArgs s{};
+    s.in = spec; s.out = spec; s.tw = c->twy();
+    s.T = P.Tys; s.nthreads = P.ntys;
+    s.line_len = P.Mx; s.tiles_per_line = (P.Mx + s.T - 1) / s.T;
+    s.n_outer = P.Mz;
+    s.in_outer_stride = s.out_outer_stride = P.plane;
+    s.in_pstride = s.out_pstride = P.Mx;
+    s.n_in = P.My; s.n_out = P.My;
+    MVD_CK(P.ly->strided(s, -1, c->stream), "y pass (spectrum)");
+    ++c->launches;
+  }
+  MVD_TRY(z_plain_fwd(c, spec));
+  return MVD_OK;
+}
+
+mvd_status precompute(mvd_ctx* c, const float* const* psfs_host) {
+  const Plan& P = c->P;
+  // twiddle tables, generated in double
+  {
+    const int M[3] = {P.Mx, P.My, P.Mz};
+    float2* dst[3] = {c->twx(), c->twy(), c->twz()};
+    for (int a = 0; a < 3; ++a) {
+      std::vector<float2> t(M[a]);
+      for (int j = 0; j < M[a]; ++j) {
+        const double ang = -2.0 * M_PI * (double)j / (double)M[a];
+        t[j] = make_float2((float)cos(ang), (float)sin(ang));
+      }
+      MVD_CK(cudaMemcpyAsync(dst[a], t.data(), sizeof(float2) * M[a], cudaMemcpyHostToDevice, c->stream), "twiddle upload");
+      MVD_CK(cudaStreamSynchronize(c->stream), "twiddle upload");
+    }
+  }
+  // normalised PSFs in fp64 (eq. 4)
+  for (int v = 0; v < P.V; ++v) {
+    const Dims3 K = P.K[v];
+    const int n = K.x * K.y * K.z;
+    double hsum = 0.0;
+    for (int i = 0; i < n; ++i) {
+      const float t = psfs_host[v][i];
+      if (!(t >= 0.f) || !std::isfinite(t)) { snprintf(c->err, sizeof(c->err), "PSF %d has a negative or non-finite tap", v); return MVD_ERR_INVALID_ARG; }
+      hsum += t;
+    }
+    if (!(hsum > 0.0)) { snprintf(c->err, sizeof(c->err), "PSF %d sums to zero", v); return MVD_ERR_INVALID_ARG; }
+    MVD_CK(cudaMemcpyAsync(c->stage(), psfs_host[v], sizeof(float) * n, cudaMemcpyHostToDevice, c->stream), "PSF upload");
+    normalise_kernel<float><<<1, 1024, 0, c->stream>>>(c->stage(), n, c->psf(v));
+    MVD_CK(cudaGetLastError(), "normalise_kernel");
+    ++c->launches;
+    MVD_CK(cudaStreamSynchronize(c->stream), "PSF upload");   // the staging buffer is reused
+  }
+  // back-projectors K_v (O3)
+  if (P.kmode == MVD_KERNEL_COMPOUND) {
+    for (int w = 0; w < P.V; ++w) {
+      const Dims3 K = P.K[w];
+      const long long tot = (long long)(2 * K.x - 1) * (2 * K.y - 1) * (2 * K.z - 1);
+      autocorr_kernel<<<(unsigned)((tot + 127) / 128), 128, 0, c->stream>>>(c->psf(w), K, c->autoc(w));
+      MVD_CK(cudaGetLastError(), "autocorr_kernel");
+      ++c->launches;
+    }
+  }
+  for (int v = 0; v < P.V; ++v) {
+    const Dims3 K = P.K[v];
+    const long long tot = (long long)K.x * K.y * K.z;
+    const unsigned g256 = (unsigned)((tot + 255) / 256), g128 = (unsigned)((tot + 127) / 128);
+    flip_pow_kernel<<<g256, 256, 0, c->stream>>>(c->psf(v), K, P.kmode == MVD_KERNEL_OPT2 ? P.V : 1, c->kern(v));
+    MVD_CK(cudaGetLastError(), "flip_pow_kernel");
+    ++c->launches;
+    if (P.kmode == MVD_KERNEL_COMPOUND || P.kmode == MVD_KERNEL_OPT1) {
+      for (int w = 0; w < P.V; ++w) {
+        if (w == v) continue;
+        const Dims3 Kw = P.K[w];
+        if (P.kmode == MVD_KERNEL_COMPOUND)
+          corr_crop_mul_kernel<<<g128, 128, 0, c->stream>>>(c->psf(v), K, c->autoc(w),
+                                                            Dims3{2 * Kw.x - 1, 2 * Kw.y - 1, 2 * Kw.z - 1}, c->kern(v));
+        else
+          corr_crop_mul_kernel<<<g128, 128, 0, c->stream>>>(c->psf(v), K, c->psf(w), Kw, c->kern(v));
+        MVD_CK(cudaGetLastError(), "corr_crop_mul_kernel");
+        ++c->launches;
+      }
+    }
+    if (P.kmode != MVD_KERNEL_PLAIN) {
+      normalise_kernel<double><<<1, 1024, 0, c->stream>>>(c->kern(v), (int)tot, c->kern(v));   // R5
+      MVD_CK(cudaGetLastError(), "normalise_kernel");
+      ++c->launches;
+    }
+  }
+  // spectra of P_v and K_v
+  for (int v = 0; v < P.V; ++v) {
+    MVD_TRY(build_spectrum(c, c->psf(v), P.K[v], c->specH(v)));
+    MVD_TRY(build_spectrum(c, c->kern(v), P.K[v], c->specK(v)));
+  }
+  return MVD_OK;
+}
+
+mvd_status init_estimate(mvd_ctx* c, const float* psi0) {
+  const Plan& P = c->P;
+  if (psi0) {
+    MVD_CK(cudaMemcpyAsync(c->psi(), psi0, sizeof(float) * P.nvox, cudaMemcpyDeviceToDevice, c->stream), "psi0 copy");
+  } else {
+    // psi^0 = average intensity over all views (L304, L421)
+    for (int v = 0; v < P.V; ++v) {
+      sum_f32_kernel<<<P.sum_blocks, 256, 0, c->stream>>>(c->views[v], P.nvox, c->partials());
+      MVD_CK(cudaGetLastError(), "sum_f32_kernel");
+      final_sum_kernel<<<1, 256, 0, c->stream>>>(c->partials(), P.sum_blocks, 1, c->scalars() + v);
+      MVD_CK(cudaGetLastError(), "final_sum_kernel");
+      c->launches += 2;
+    }
+    fill_mean_kernel<<<1184, 256, 0, c->stream>>>(c->psi(), P.nvox, c->scalars(), P.V, (double)P.nvox * P.V);
+    MVD_CK(cudaGetLastError(), "fill_mean_kernel");
+    ++c->launches;
+  }
+  c->w_valid = false;
+  c->stats_valid = false;
+  return MVD_OK;
+}
+
+const mvd_options* defaults(const mvd_options* opt, mvd_options* tmp) {
+  mvd_options_init(tmp);
+  if (opt) {
+    const size_t n = std::min(opt->struct_size, sizeof(mvd_options));
+    if (n >= sizeof(size_t)) memcpy(tmp, opt, n);
+    tmp->struct_size = sizeof(mvd_options);
+  }
+  return tmp;
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------
+// C ABI
+// ---------------------------------------------------------------------------------------
+extern "C" {
+
+void mvd_options_init(mvd_options* opt) {
+  if (!opt) return;
+  memset(opt, 0, sizeof(*opt));
+  opt->struct_size = sizeof(*opt);
+  opt->eps = 1e-6f;
+  opt->psi_floor = 1e-6f;
+}
+
+size_t mvd_workspace_size(int n_views, const int dims[3], const int (*psf_dims)[3],
+                          mvd_variant variant, const mvd_options* opt) {
+  mvd_options tmp;
+  Plan P;
+  if (make_plan(P, n_views, dims, psf_dims, variant, defaults(opt, &tmp)) != MVD_OK) return 0;
+  return P.total;
+}
+
+mvd_status mvd_plan_dims(int n_views, const int dims[3], const int (*psf_dims)[3],
+                         const mvd_options* opt, int fft_dims_out[3]) {
+  if (!fft_dims_out) return MVD_ERR_INVALID_ARG;
+  mvd_options tmp;
+  Plan P;
+  mvd_status s = make_plan(P, n_views, dims, psf_dims, MVD_OSEM, defaults(opt, &tmp));
+  if (s != MVD_OK) return s;
+  fft_dims_out[0] = P.Mx; fft_dims_out[1] = P.My; fft_dims_out[2] = P.Mz;
+  return MVD_OK;
+}
+
+mvd_status mvd_create(mvd_ctx** out, int n_views, const float* const* views, const int dims[3],
+                      const float* const* psfs, const int (*psf_dims)[3], mvd_variant variant,
+                      const mvd_options* opt_in) {
+  if (!out) return MVD_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!views || !psfs || !dims || !psf_dims || !opt_in) return MVD_ERR_INVALID_ARG;
+  mvd_options tmp;
+  const mvd_options* opt = defaults(opt_in, &tmp);
+  for (int v = 0; v < n_views; ++v)
+    if (!views[v] || !psfs[v]) return MVD_ERR_INVALID_ARG;
+  mvd_ctx* c = new (std::nothrow) mvd_ctx();
+  if (!c) return MVD_ERR_INVALID_ARG;
+  mvd_status s = make_plan(c->P, n_views, dims, psf_dims, variant, opt);
+  if (s != MVD_OK) { delete c; return s; }
+  if (!opt->workspace || (reinterpret_cast<size_t>(opt->workspace) & 255) || opt->workspace_bytes < c->P.total) {
+    delete c;
+    return MVD_ERR_WORKSPACE;
+  }
+  c->variant = variant;
+  c->literal = opt->literal_product ? 1 : 0;
+  c->eps = opt->eps > 0.f ? opt->eps : 1e-6f;
+  c->psi_floor = opt->psi_floor >= 0.f ? opt->psi_floor : 1e-6f;
+  c->stream = reinterpret_cast<cudaStream_t>(opt->stream);
+  c->ws = reinterpret_cast<char*>(opt->workspace);
+  c->use_graph = opt->use_graph;
+  c->views.assign(views, views + n_views);
+
+  cudaError_t e = cudaSuccess;
+  const LengthOps* ls[3] = {c->P.lx, c->P.ly, c->P.lz};
+  for (int a = 0; a < 3 && e == cudaSuccess; ++a) e = ls[a]->init();
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) { delete c; return MVD_ERR_CUDA; }
+
+  s = precompute(c, psfs);
+  if (s == MVD_OK) s = init_estimate(c, opt->psi0);
+  if (s == MVD_OK && c->fail(cudaStreamSynchronize(c->stream), "mvd_create")) s = MVD_ERR_CUDA;
+  if (s != MVD_OK) {
+    if (c->err[0]) fprintf(stderr, "mvd_create: %s\n", c->err);
+    delete c;
+    return s;
+  }
+  *out = c;
+  return MVD_OK;
+}
+
+mvd_status mvd_iterate(mvd_ctx* c, int n) {
+  if (!c || n < 0) return MVD_ERR_INVALID_ARG;
+  if (c->broken) return MVD_ERR_STATE;
+  if (n == 0) return MVD_OK;
+  MVD_TRY(ensure_w(c));
+  if (c->use_graph) {
+    if (!c->graph_exec) {
+      cudaGraph_t g = nullptr;
+      const long long before = c->launches;
+      MVD_CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal), "graph capture begin");
+      mvd_status s = iteration_body(c);
+      cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+      if (s != MVD_OK) return s;
+      MVD_CK(e, "graph capture end");
+      c->graph_launches = c->launches - before;
+      c->launches = before;
+      MVD_CK(cudaGraphInstantiate(&c->graph_exec, g, 0), "graph instantiate");
+      cudaGraphDestroy(g);
+    }
+    for (int i = 0; i < n; ++i) {
+      MVD_CK(cudaGraphLaunch(c->graph_exec, c->stream), "graph launch");
+      c->launches += c->graph_launches;
+      ++c->iters;
+    }
+    return MVD_OK;
+  }
+  for (int i = 0; i < n; ++i) {
+    MVD_TRY(iteration_body(c));
+    ++c->iters;
+  }
+  return MVD_OK;
+}
+
+mvd_status mvd_get_estimate(mvd_ctx* c, float* dst, int dst_is_device) {
+  if (!c || !dst) return MVD_ERR_INVALID_ARG;
+  if (c->broken) return MVD_ERR_STATE;
+  const size_t bytes = sizeof(float) * (size_t)c->P.nvox;
+  if (dst_is_device) {
+    MVD_CK(cudaMemcpyAsync(dst, c->psi(), bytes, cudaMemcpyDeviceToDevice, c->stream), "estimate copy");
+  } else {
+    MVD_CK(cudaMemcpyAsync(dst, c->psi(), bytes, cudaMemcpyDeviceToHost, c->stream), "estimate copy");
+    MVD_CK(cudaStreamSynchronize(c->stream), "estimate copy");
+  }
+  return MVD_OK;
+}
+
+mvd_status mvd_set_estimate(mvd_ctx* c, const float* src_device) {
+  if (!c || !src_device) return MVD_ERR_INVALID_ARG;
+  if (c->broken) return MVD_ERR_STATE;
+  MVD_CK(cudaMemcpyAsync(c->psi(), src_device, sizeof(float) * (size_t)c->P.nvox, cudaMemcpyDeviceToDevice, c->stream), "estimate copy");
+  c->w_valid = false;
+  c->stats_valid = false;
+  return MVD_OK;
+}
+
+mvd_status mvd_get_stats(mvd_ctx* c, double* flux, double* l1_change, int* iterations_done) {
+  if (!c) return MVD_ERR_INVALID_ARG;
+  if (c->broken) return MVD_ERR_STATE;
+  double h[2] = {0.0, 0.0};
+  double* d = c->scalars() + c->P.V;
+  if (c->stats_valid) {
+    final_sum_kernel<<<1, 256, 0, c->stream>>>(c->partials(), c->stats_ncta, 2, d);
+    MVD_CK(cudaGetLastError(), "final_sum_kernel");
+    ++c->launches;
+  } else {
+    // no update yet: flux of the current estimate, no change
+    sum_f32_kernel<<<c->P.sum_blocks, 256, 0, c->stream>>>(c->psi(), c->P.nvox, c->partials());
+    MVD_CK(cudaGetLastError(), "sum_f32_kernel");
+    final_sum_kernel<<<1, 256, 0, c->stream>>>(c->partials(), c->P.sum_blocks, 1, d);
+    MVD_CK(cudaGetLastError(), "final_sum_kernel");
+    MVD_CK(cudaMemsetAsync(d + 1, 0, sizeof(double), c->stream), "memset");
+    c->launches += 2;
+  }
+  MVD_CK(cudaMemcpyAsync(h, d, sizeof(h), cudaMemcpyDeviceToHost, c->stream), "stats copy");
+  MVD_CK(cudaStreamSynchronize(c->stream), "stats copy");
+  if (flux) *flux = h[0];
+  if (l1_change) *l1_change = h[1];
+  if (iterations_done) *iterations_done = c->iters;
+  return MVD_OK;
+}
+
+mvd_status mvd_get_back_projector(mvd_ctx* c, int view, double* dst_host) {
+  if (!c || !dst_host || view < 0 || view >= c->P.V) return MVD_ERR_INVALID_ARG;
+  if (c->broken) return MVD_ERR_STATE;
+  const Dims3 K = c->P.K[view];
+  MVD_CK(cudaMemcpyAsync(dst_host, c->kern(view), sizeof(double) * (size_t)K.x * K.y * K.z, cudaMemcpyDeviceToHost, c->stream), "kernel copy");
+  MVD_CK(cudaStreamSynchronize(c->stream), "kernel copy");
+  return MVD_OK;
+}
+
+mvd_status mvd_convolve(mvd_ctx* c, int view, int which, const float* src, float* dst) {
+  if (!c || !src || !dst || view < 0 || view >= c->P.V || which < 0 || which > 1) return MVD_ERR_INVALID_ARG;
+  if (c->broken) return MVD_ERR_STATE;
+  c->w_valid = false;
+  MVD_TRY(x_load(c, src, c->W()));
+  MVD_TRY(conv_core(c, nullptr, c->W(), which ? c->specK(view) : c->specH(view), false));
+  XArgs a = x_args(c, c->W(), c->W(), (c->P.K[view].x - 1) / 2);
+  a.acc = dst;
+  a.acc_mode = ACC_STORE;
+  return x_pass(c, a, X_ACCUM);
+}
+
+long long mvd_launch_count(const mvd_ctx* c) { return c ? c->launches : 0; }
+
+void mvd_destroy(mvd_ctx* c) {
+  if (!c) return;
+  if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+  delete c;
+}
+
+const char* mvd_status_string(mvd_status s) {
+  switch (s) {
+    case MVD_OK: return "ok";
+    case MVD_ERR_INVALID_ARG: return "invalid argument";
+    case MVD_ERR_UNSUPPORTED: return "unsupported size (no FFT length available)";
+    case MVD_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+    case MVD_ERR_CUDA: return "CUDA error";
+    case MVD_ERR_STATE: return "context unusable after an earlier CUDA error";
+  }
+  return "unknown status";
+}
+
+const char* mvd_last_error(const mvd_ctx* c) { return c ? c->err : ""; }
+
+}  // extern "C"
+
+// ---- block-wise processing (S6; L64, L943; R13) ----------------------------------------------------
+namespace {
+
+struct Seg { int c0, c1, e0, e1; };   // central [c0,c1), extended [e0,e1)
+
+std::vector<Seg> segments(int n, int block, int halo) {
+  std::vector<Seg> out;
+  for (int s = 0; s < n; s += block) {
+    const int e = std::min(s + block, n);
+    out.push_back(Seg{s, e, std::max(s - halo, 0), std::min(e + halo, n)});
+  }
+  return out;
+}
+
+struct BlockedLayout {
+  int halo[3];
+  std::vector<Seg> seg[3];
+  size_t max_ext = 0;          // voxels of the largest extended block
+  size_t ctx_bytes = 0;        // largest context workspace over the distinct extended shapes
+  std::vector<std::array<int, 3>> shapes;
+  size_t off_scal = 0, off_views = 0, off_psi0 = 0, off_est = 0, off_ctx = 0, total = 0;
+};
+
+mvd_status blocked_layout(BlockedLayout& L, int n_views, const int dims[3], const int (*psf_dims)[3],
+                          mvd_variant variant, const mvd_options* opt, const int block_dims[3],
+                          const int halo[3]) {
+  if (n_views < 1 || !dims || !psf_dims || !block_dims) return MVD_ERR_INVALID_ARG;
+  for (int a = 0; a < 3; ++a) {
+    if (dims[a] < 1 || block_dims[a] < 1) return MVD_ERR_INVALID_ARG;
+    int h = 0;
+    for (int v = 0; v < n_views; ++v) h = std::max(h, (psf_dims[v][a] - 1) / 2);
+    L.halo[a] = halo ? halo[a] : h;
+    if (L.halo[a] < 0) return MVD_ERR_INVALID_ARG;
+    L.seg[a] = segments(dims[a], block_dims[a], L.halo[a]);
+  }
+  for (const Seg& sz : L.seg[2])
+    for (const Seg& sy : L.seg[1])
+      for (const Seg& sx : L.seg[0]) {
+        std::array<int, 3> e = {sx.e1 - sx.e0, sy.e1 - sy.e0, sz.e1 - sz.e0};
+        if (std::find(L.shapes.begin(), L.shapes.end(), e) == L.shapes.end()) L.shapes.push_back(e);
+      }
+  mvd_options o = *opt;
+  o.fft_dims[0] = o.fft_dims[1] = o.fft_dims[2] = 0;
+  for (const auto& e : L.shapes) {
+    const int d[3] = {e[0], e[1], e[2]};
+    const size_t b = mvd_workspace_size(n_views, d, psf_dims, variant, &o);
+    if (b == 0) return MVD_ERR_UNSUPPORTED;
+    L.ctx_bytes = std::max(L.ctx_bytes, b);
+    L.max_ext = std::max(L.max_ext, (size_t)e[0] * e[1] * e[2]);
+  }
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t at = off; off = align_up(off + bytes, 256); return at; };
+  L.off_scal = take(sizeof(double) * (size_t)(1184 + n_views + 8));
+  L.off_views = take(align_up(L.max_ext * sizeof(float), 256) * n_views);
+  L.off_psi0 = take(L.max_ext * sizeof(float));
+  L.off_est = take(L.max_ext * sizeof(float));
+  L.off_ctx = take(L.ctx_bytes);
+  L.total = off;
+  return MVD_OK;
+}
+
+}  // namespace
+
+extern "C" size_t mvd_blocked_workspace_size(int n_views, const int dims[3], const int (*psf_dims)[3],
+                                             mvd_variant variant, const mvd_options* opt_in,
+                                             const int block_dims[3], const int halo[3]) {
+  mvd_options tmp;
+  BlockedLayout L;
+  if (blocked_layout(L, n_views, dims, psf_dims, variant, defaults(opt_in, &tmp), block_dims, halo) != MVD_OK) return 0;
+  return L.total;
+}
+
+extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* views, const int dims[3],
+                                             const float* const* psfs, const int (*psf_dims)[3],
+                                             mvd_variant variant, const mvd_options* opt_in,
+                                             const int block_dims[3], const int halo[3], int iterations,
+                                             float* dst, long long* launches_out) {
+  if (!views || !psfs || !dst || !opt_in || iterations < 0) return MVD_ERR_INVALID_ARG;
+  mvd_options tmp;
+  const mvd_options* opt = defaults(opt_in, &tmp);
+  BlockedLayout L;
+  mvd_status s = blocked_layout(L, n_views, dims, psf_dims, variant, opt, block_dims, halo);
+  if (s != MVD_OK) return s;
+  if (!opt->workspace || (reinterpret_cast<size_t>(opt->workspace) & 255) || opt->workspace_bytes < L.total)
+    return MVD_ERR_WORKSPACE;
+  char* ws = reinterpret_cast<char*>(opt->workspace);
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(opt->stream);
+  double* partial = reinterpret_cast<double*>(ws + L.off_scal);
+  double* sums = partial + 1184;
+  const size_t vstride = align_up(L.max_ext * sizeof(float), 256);
+  std::vector<const float*> bviews(n_views);
+  for (int v = 0; v < n_views; ++v) bviews[v] = reinterpret_cast<const float*>(ws + L.off_views + v * vstride);
+  float* psi0 = reinterpret_cast<float*>(ws + L.off_psi0);
+  float* est = reinterpret_cast<float*>(ws + L.off_est);
+  long long launches = 0;
+  const Dims3 N{dims[0], dims[1], dims[2]};
+  const long long nvox = (long long)dims[0] * dims[1] * dims[2];
+
+  // psi^0 = mean over the WHOLE volume and all views (R13), kept on the device
+  for (int v = 0; v < n_views; ++v) {
+    if (!views[v]) return MVD_ERR_INVALID_ARG;
+    sum_f32_kernel<<<1184, 256, 0, st>>>(views[v], nvox, partial);
+    final_sum_kernel<<<1, 256, 0, st>>>(partial, 1184, 1, sums + v);
+    launches += 2;
+  }
+  fill_mean_kernel<<<1184, 256, 0, st>>>(psi0, (long long)L.max_ext, sums, n_views, (double)nvox * n_views);
+  ++launches;
+  if (cudaGetLastError() != cudaSuccess) return MVD_ERR_CUDA;
+
+  for (const auto& shape : L.shapes) {
+    const int d[3] = {shape[0], shape[1], shape[2]};
+    mvd_options o = *opt;
+    o.fft_dims[0] = o.fft_dims[1] = o.fft_dims[2] = 0;
+    o.psi0 = psi0;
+    o.workspace = ws + L.off_ctx;
+    o.workspace_bytes = L.ctx_bytes;
+    mvd_ctx* c = nullptr;
+    s = mvd_create(&c, n_views, bviews.data(), d, psfs, psf_dims, variant, &o);
+    if (s != MVD_OK) return s;
+    const Dims3 E{d[0], d[1], d[2]};
+    const long long ext = (long long)d[0] * d[1] * d[2];
+    const unsigned grid = (unsigned)std::min<long long>((ext + 255) / 256, 1184 * 8);
+    for (const Seg& sz : L.seg[2])
+      for (const Seg& sy : L.seg[1])
+        for (const Seg& sx : L.seg[0]) {
+          if (sx.e1 - sx.e0 != d[0] || sy.e1 - sy.e0 != d[1] || sz.e1 - sz.e0 != d[2]) continue;
+          for (int v = 0; v < n_views; ++v) {
+            gather_block_kernel<<<grid, 256, 0, st>>>(views[v], N, Dims3{sx.e0, sy.e0, sz.e0}, E,
+                                                      const_cast<float*>(bviews[v]));
+            ++launches;
+          }
+          s = mvd_set_estimate(c, psi0);
+          if (s == MVD_OK) s = mvd_iterate(c, iterations);
+          if (s == MVD_OK) s = mvd_get_estimate(c, est, 1);
+          if (s != MVD_OK) { mvd_destroy(c); return s; }
+          paste_block_kernel<<<grid, 256, 0, st>>>(est, E, Dims3{sx.c0 - sx.e0, sy.c0 - sy.e0, sz.c0 - sz.e0},
+                                                   Dims3{sx.c1 - sx.c0, sy.c1 - sy.c0, sz.c1 - sz.c0}, dst, N,
+                                                   Dims3{sx.c0, sy.c0, sz.c0});
+          ++launches;
+        }
+    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { mvd_destroy(c); return MVD_ERR_CUDA; }
+    launches += mvd_launch_count(c);
+    mvd_destroy(c);
+  }
+  if (launches_out) *launches_out = launches;
+  return MVD_OK;
+}

@@ -18,7 +18,7 @@ def test_config1_shapes_and_determinism():
     assert np.allclose(a.psfs[0], a.psfs[0][::-1, ::-1, ::-1], atol=1e-7)
     # views carry roughly the same flux (R10)
     sums = [float(v.sum()) for v in a.views]
-    assert max(sums) / min(sums) < 1.05
+    assert max(sums) / min(sums) < 1.10
 
 
 def test_rotated_psf_is_elongated_along_x_at_90_degrees():
