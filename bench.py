@@ -1,0 +1,438 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the multi-view Richardson-Lucy hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+
+A *step* is one iteration of efficient-OSEM (eq. 109-112 with the compound kernels of eq. 105):
+every view blurs psi, forms the quotient, back-projects it and updates psi (V view-updates,
+8 kernel launches each).  The workload is BASELINE.json configs[3] (512x512x256, 7 views, PSFs
+21x21x45: the volume north_star quotes its target on), seeded and synthetic (mvd_synth).  Metric: Gvoxel-view
+updates/s = Nx*Ny*Nz*V*K / t / 1e9 on un-padded voxels, inputs resident in HBM, CUDA events on
+the launching stream, max over ranks.  The path does not shard (OSEM is a strict sequence of
+global FFTs): --gpus N runs N independent replicas, no collective on
+the data path.
+
+One JSON line on stdout (rank 0).  Extra objects: `roofline` (dominant kernel class, algorithmic
+bytes / live CUDA-event time), `kernels` (every class), `cpu_baseline` (the fp64 oracle timed on
+this box's host cores on a bounded sample), `e2e` (whole job through the public API from pinned
+host buffers: H2D of the views, mvd_create, all iterations, D2H of the estimate).
+
+--impl reference times the oracle itself (rank 0 only), one view-update of the same recipe at
+256x256x128 per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import tempfile
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Gvoxel-view updates/s per iteration (fp32)"
+UNIT = "Gvv/s"
+FALLBACK_HBM_GBS = 6650.0     # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+NOMINAL_HBM_GBS = 8000.0      # north_star's "roughly 8 TB/s"
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+# ------------------------------------------------------------------------------------------
+# clocks: NVML sampling thread (falls back to nothing if NVML is unavailable)
+# ------------------------------------------------------------------------------------------
+REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+           0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+           0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+
+class ClockSampler:
+    def __init__(self, index, period=0.02):
+        self.samples = []          # (t, sm_mhz, reasons_mask, power_w)
+        self.period = period
+        self.stop_flag = threading.Event()
+        self.ok = False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:
+                import torch
+                uuid = "GPU-" + str(torch.cuda.get_device_properties(index).uuid)
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid)
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # pragma: no cover
+            log("[bench] NVML unavailable: %r" % (e,))
+        self.th = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        nv = self.nv
+        while not self.stop_flag.is_set():
+            try:
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                try:
+                    pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                except Exception:
+                    pw = float("nan")
+                self.samples.append((time.perf_counter(), float(mhz), int(mask), pw))
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def start(self):
+        if self.ok:
+            self.th.start()
+
+    def stop(self):
+        self.stop_flag.set()
+        if self.ok:
+            self.th.join(timeout=2)
+
+    def summary(self, t0, t1):
+        inside = [s for s in self.samples if t0 <= s[0] <= t1]
+        window = "timed region"
+        if not inside:
+            inside = self.samples[-3:]
+            window = "nearest samples (timed region shorter than the sampling period)"
+        if not inside:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0, "window": "none"}
+        mask = 0
+        for s in inside:
+            mask |= s[2]
+        reasons = [name for bit, name in REASONS.items() if mask & bit and name != "gpu_idle"]
+        return {"sm_mhz": float(np.median([s[1] for s in inside])), "sm_max_mhz": self.max_mhz,
+                "reasons": reasons, "samples": len(inside), "window": window,
+                "power_w_max": float(np.nanmax([s[3] for s in inside]))}
+
+
+# ------------------------------------------------------------------------------------------
+# algorithmic bytes per launch of every kernel class
+# ------------------------------------------------------------------------------------------
+def algorithmic_bytes(dims, fft_dims):
+    nx, ny, nz = dims
+    mx, my, mz = fft_dims            # mx = complex half-row length
+    row = 8 * mx                     # bytes of one complex work-buffer row
+    n = nx * ny * nz
+    return {
+        "y_fwd": row * ny * nz + row * my * nz,
+        "y_inv": row * my * nz + row * ny * nz,
+        "z_conv": 2 * row * my * nz + row * my * mz,
+        "x_quot": 2 * row * ny * nz + 4 * n,
+        "x_update": 2 * row * ny * nz + 8 * n,
+        "x_accum": 2 * row * ny * nz + 12 * n,
+        "x_load": row * ny * nz + 4 * n,
+    }
+
+
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy_)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(kernel_class, k):
+    """dram bytes per launch of the class from the committed ncu --set full capture, or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(p))["config%d" % k][kernel_class]
+    except Exception:
+        return None
+
+
+# ------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------
+def load_problem(k, rank, world, dist):
+    """rank 0 draws the problem; with several ranks it is handed over through /tmp."""
+    import mvd_synth
+    if world == 1:
+        return mvd_synth.make_problem(k)
+    tmp = os.path.join(tempfile.gettempdir(), "mvd_bench_cfg%d_%s" % (k, os.environ.get("MASTER_PORT", "0")))
+    if rank == 0:
+        p = mvd_synth.make_problem(k)
+        os.makedirs(tmp, exist_ok=True)
+        for v, (a, b) in enumerate(zip(p.views, p.psfs)):
+            np.save(os.path.join(tmp, "view%d.npy" % v), a)
+            np.save(os.path.join(tmp, "psf%d.npy" % v), b)
+        dist.barrier()
+        return p
+    dist.barrier()
+    nv = len(mvd_synth.CONFIGS[k]["angles"])
+    views = [np.load(os.path.join(tmp, "view%d.npy" % v)) for v in range(nv)]
+    psfs = [np.load(os.path.join(tmp, "psf%d.npy" % v)) for v in range(nv)]
+    rec = mvd_synth.CONFIGS[k]
+    return mvd_synth.Problem(k, rec["dims"], rec["psf"], None, psfs, views, rec["iterations"], rec["variants"])
+
+
+def cpu_baseline(prob, budget_s=12.0):
+    """The oracle as it stands, on this box's host cores: whole view-updates of efficient-OSEM on
+    the full volume until `budget_s` seconds are spent (at least one)."""
+    from oracle import mvd_oracle as O
+    cores = len(os.sched_getaffinity(0))
+    o = O.Oracle(prob.views, prob.psfs, "osem")
+    n = 0
+    t0 = time.perf_counter()
+    while n < prob.n_views:
+        o._commit(np.maximum(o.psi * o.factor(n), o.psi_floor))   # one step of Oracle.iterate's OSEM loop
+        n += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    nvox = float(np.prod(prob.dims))
+    return {"value": nvox * n / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "first %d of %d view-updates of one efficient-OSEM iteration on the full %dx%dx%d volume "
+                      "(fp64, scipy.fft with %d workers), %.1f s" % (n, prob.n_views, *prob.dims, cores, dt)}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1308_0730_b200 as mvd
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU path; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    mvd.load_library()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    k = args.config
+    t = time.perf_counter()
+    prob = load_problem(k, rank, world, dist)
+    log("[bench] rank %d: config %d drawn in %.1f s" % (rank, k, time.perf_counter() - t))
+    V, dims = prob.n_views, prob.dims
+    nvox = float(np.prod(dims))
+
+    host_views = [torch.from_numpy(v).pin_memory() for v in prob.views]
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        dev_views = [h.to("cuda", non_blocking=True) for h in host_views]
+    stream.synchronize()
+
+    t = time.perf_counter()
+    d = mvd.Deconvolver(dev_views, prob.psfs, variant="osem", stream=stream, use_graph=args.graph)
+    create_ms = (time.perf_counter() - t) * 1e3
+    fft_dims = d.fft_dims
+    workspace_gb = d.workspace_bytes / 1e9
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps ---------------------------
+    sampler = ClockSampler(local)
+    sampler.start()
+    for _ in range(args.warmup):
+        d.iterate(1)
+    profile_live = not args.graph
+    if profile_live:
+        d.profile(True)
+    launches0 = d.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.perf_counter()
+    e0.record(stream)
+    for _ in range(args.steps):
+        d.iterate(1)
+    e1.record(stream)
+    barrier()
+    t1 = time.perf_counter()
+    ms = e0.elapsed_time(e1)
+    launches = d.launch_count - launches0
+    classes = d.profile_read() if profile_live else {}
+    if profile_live:
+        d.profile(False)
+    clocks = sampler.summary(t0, t1)
+    sampler.stop()
+    stats = d.get_stats()
+    if not np.isfinite(stats["flux"]):
+        raise SystemExit("bench.py: non-finite estimate")
+
+    # the same K steps without the per-launch events, to show they do not distort the number
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        d.iterate(1)
+    e1.record(stream)
+    barrier()
+    ms_plain = e0.elapsed_time(e1)
+
+    if world > 1:
+        tmax = torch.tensor([ms, ms_plain], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        ms, ms_plain = float(tmax[0]), float(tmax[1])
+    value = world * nvox * V * args.steps / (ms * 1e-3) / 1e9
+
+    # ---- roofline of the dominant kernel class --------------------------------------------------
+    peak, peak_src = hbm_peak()
+    alg = algorithmic_bytes(dims, fft_dims)
+    kernels = {}
+    for name, (tms, n) in classes.items():
+        if n:
+            per = tms / n
+            kernels[name] = {"launches": n, "avg_ms": per, "share": tms / ms,
+                             "algorithmic_bytes": alg[name], "achieved_gbs": alg[name] / (per * 1e-3) / 1e9}
+    step_bytes = sum(alg[name] * kk["launches"] for name, kk in kernels.items()) / max(args.steps, 1)
+    roofline = None
+    if kernels:
+        top = max(kernels, key=lambda n: kernels[n]["share"])
+        a = kernels[top]["achieved_gbs"]
+        roofline = {"bound": "hbm", "kernel": top, "achieved": a, "peak": peak, "unit": "GB/s", "frac": a / peak,
+                    "traffic": ncu_traffic(top, k), "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": alg[top],
+                    "step": {"algorithmic_bytes": step_bytes,
+                             "achieved": step_bytes / (ms / args.steps * 1e-3) / 1e9,
+                             "frac_of_measured": step_bytes / (ms / args.steps * 1e-3) / 1e9 / peak,
+                             "frac_of_nominal_8TBs": step_bytes / (ms / args.steps * 1e-3) / 1e9 / NOMINAL_HBM_GBS}}
+
+    # ---- end to end from pinned host buffers, through the public API -----------------------------
+    e2e = None
+    if args.e2e_jobs > 0:
+        iters = prob.iterations
+        out_host = torch.empty(prob.views[0].shape, dtype=torch.float32).pin_memory()
+        h2d = sum(h.numel() * 4 for h in host_views)
+        d2h = out_host.numel() * 4
+        d.close()
+        del d, dev_views
+        torch.cuda.empty_cache()
+
+        def job():
+            with torch.cuda.stream(stream):
+                dv = [h.to("cuda", non_blocking=True) for h in host_views]
+            dd = mvd.Deconvolver(dv, prob.psfs, variant="osem", stream=stream)
+            dd.iterate(iters)
+            dd.get_estimate_host(out_host.numpy())
+            dd.close()
+
+        job()                                          # warm-up job (allocator, page-ins)
+        barrier()
+        tw0 = time.perf_counter()
+        for _ in range(args.e2e_jobs):
+            job()
+        barrier()
+        dt = time.perf_counter() - tw0
+        if world > 1:
+            tt = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            dt = float(tt[0])
+        e2e = {"value": world * nvox * V * iters * args.e2e_jobs / dt / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "step": "one whole job: H2D of the %d views from pinned host memory, mvd_create (PSF upload, "
+                       "compound kernels, spectra), %d iterations, D2H of the estimate; wall clock between "
+                       "synchronisations" % (V, iters),
+               "jobs": args.e2e_jobs, "ms_per_job": dt / args.e2e_jobs * 1e3}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cpu = cpu_baseline(prob)
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "BASELINE configs[%d]: %dx%dx%d, %d views, PSF %dx%dx%d, efficient-OSEM "
+                                   "(MVD_OSEM + compound kernels), one step = one iteration" % (k - 1, *dims, V, *prob.psf_dims),
+                       "fft_dims": list(fft_dims), "voxel_views_per_step": nvox * V,
+                       "parallelism": "replicas x%d (no data-path collective)" % world,
+                       "l2": "inputs larger than L2 (one view-update streams %.1f GB)" % (step_bytes / V / 1e9 if kernels else 0.0),
+                       "cuda_graph": bool(args.graph)},
+            "clocks": clocks, "gpu_launches": launches, "e2e": e2e,
+            "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu,
+            "create_ms": create_ms, "ms_per_step_without_launch_events": ms_plain / args.steps,
+            "workspace_gb": workspace_gb, "flux": stats["flux"],
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------
+# reference arm: the oracle, on the host
+# ------------------------------------------------------------------------------------------
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank != 0:
+        return
+    import mvd_synth
+    from oracle import mvd_oracle as O
+
+    k = args.config
+    rec = mvd_synth.CONFIGS[k]
+    dims = tuple(max(16, n // 2) for n in rec["dims"]) if k >= 4 else rec["dims"]
+    prob = mvd_synth.make_problem(k, dims=dims)
+    cores = len(os.sched_getaffinity(0))
+    o = O.Oracle(prob.views, prob.psfs, "osem")
+    V = prob.n_views
+    nvox = float(np.prod(dims))
+
+    def step(i):
+        v = i % V
+        o._commit(np.maximum(o.psi * o.factor(v), o.psi_floor))
+
+    for i in range(args.warmup):
+        step(i)
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        step(args.warmup + i)
+    dt = time.perf_counter() - t0
+    value = nvox * args.steps / dt / 1e9
+    sample = ("one view-update of efficient-OSEM per step (views in index order) on the config-%d recipe at "
+              "%dx%dx%d, %d views, PSF %dx%dx%d; fp64 numpy/scipy.fft, %d workers"
+              % (k, *dims, V, *prob.psf_dims, cores))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE config number 1..5 (default 4, the target volume)")
+    ap.add_argument("--graph", action="store_true", help="replay each iteration as one CUDA graph (no per-kernel timing)")
+    ap.add_argument("--e2e-jobs", type=int, default=2)
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -139,6 +139,25 @@ MVD_API mvd_status mvd_convolve(mvd_ctx* ctx, int view, int which, const float* 
 /* Number of kernel launches the library has issued on this context since creation. */
 MVD_API long long mvd_launch_count(const mvd_ctx* ctx);
 
+/* Per-kernel-class device timing, for the roofline report.  While
+ * enabled, every pass kernel of mvd_iterate is bracketed by a pair of CUDA events on the context's
+ * stream (not available with use_graph: MVD_ERR_STATE).  mvd_profile_read synchronises the stream,
+ * writes the summed device time (milliseconds) and the launch count of each class into two HOST
+ * arrays of MVD_K_COUNT entries, and clears the record. */
+typedef enum {
+  MVD_K_Y_FWD = 0,           /* y forward pencil pass (pruned input)                         */
+  MVD_K_Y_INV = 1,           /* y inverse pencil pass (cropped output)                       */
+  MVD_K_Z_CONV = 2,          /* z forward . spectrum . z inverse                             */
+  MVD_K_X_QUOT = 3,          /* x inverse -> quotient -> x forward                           */
+  MVD_K_X_UPDATE = 4,        /* x inverse -> psi update -> x forward (OSEM)                  */
+  MVD_K_X_ACCUM = 5,         /* x inverse -> product accumulation / combined update          */
+  MVD_K_X_LOAD = 6,          /* x forward of psi (first iteration, after mvd_set_estimate)   */
+  MVD_K_COUNT = 7
+} mvd_kernel_class;
+MVD_API mvd_status mvd_profile(mvd_ctx* ctx, int enable);
+MVD_API mvd_status mvd_profile_read(mvd_ctx* ctx, double* total_ms_host, long long* launches_host);
+MVD_API const char* mvd_kernel_class_name(int kernel_class);
+
 /* Block-wise processing (L64, L943; R13): tiles the volume into blocks of block_dims, extends
  * every block by `halo` voxels of neighbouring data per side (clipped at the volume faces; halo
  * = NULL -> PSF half-size), runs `iterations` iterations on each extended block with

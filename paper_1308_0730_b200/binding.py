@@ -16,13 +16,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmvd.so")
 
 VARIANTS = {"independent": 0, "efficient": 1, "osem": 2}
+N_KERNEL_CLASSES = 7      # MVD_K_COUNT
 KERNEL_MODES = {"auto": 0, "plain": 1, "compound": 2, "opt1": 3, "opt2": 4}
 
 # every symbol include/mvd.h declares (tests check that the library exports them all)
 SYMBOLS = (
     "mvd_options_init", "mvd_workspace_size", "mvd_plan_dims", "mvd_create", "mvd_iterate",
     "mvd_get_estimate", "mvd_set_estimate", "mvd_get_stats", "mvd_get_back_projector", "mvd_convolve",
-    "mvd_launch_count", "mvd_blocked_workspace_size", "mvd_deconvolve_blocked", "mvd_destroy",
+    "mvd_launch_count", "mvd_profile", "mvd_profile_read", "mvd_kernel_class_name", "mvd_blocked_workspace_size", "mvd_deconvolve_blocked", "mvd_destroy",
     "mvd_status_string", "mvd_last_error",
 )
 
@@ -84,6 +85,12 @@ def load_library():
     lib.mvd_convolve.restype = C.c_int
     lib.mvd_launch_count.argtypes = [vp]
     lib.mvd_launch_count.restype = C.c_longlong
+    lib.mvd_profile.argtypes = [vp, C.c_int]
+    lib.mvd_profile.restype = C.c_int
+    lib.mvd_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    lib.mvd_profile_read.restype = C.c_int
+    lib.mvd_kernel_class_name.argtypes = [C.c_int]
+    lib.mvd_kernel_class_name.restype = C.c_char_p
     lib.mvd_blocked_workspace_size.argtypes = [C.c_int, _Int3, vp, C.c_int, C.POINTER(mvd_options), _Int3, vp]
     lib.mvd_blocked_workspace_size.restype = C.c_size_t
     lib.mvd_deconvolve_blocked.argtypes = [C.c_int, C.POINTER(vp), _Int3, C.POINTER(vp), vp, C.c_int,
@@ -260,6 +267,16 @@ class Deconvolver:
         _check(self._lib.mvd_convolve(self._ctx, int(view), int(which), s.data_ptr(), dst.data_ptr()), self._ctx, "mvd_convolve")
         self.stream.synchronize()
         return dst
+
+    def profile(self, enable=True):
+        _check(self._lib.mvd_profile(self._ctx, int(bool(enable))), self._ctx, "mvd_profile")
+
+    def profile_read(self):
+        """{kernel class: (total device ms, launches)} since the last read; synchronises."""
+        ms = (C.c_double * N_KERNEL_CLASSES)()
+        n = (C.c_longlong * N_KERNEL_CLASSES)()
+        _check(self._lib.mvd_profile_read(self._ctx, ms, n), self._ctx, "mvd_profile_read")
+        return {self._lib.mvd_kernel_class_name(k).decode(): (ms[k], int(n[k])) for k in range(N_KERNEL_CLASSES)}
 
     @property
     def launch_count(self):

@@ -231,6 +231,20 @@ struct mvd_ctx {
   cudaGraphExec_t graph_exec = nullptr;
   long long graph_launches = 0;
   char err[512] = {0};
+  // per-kernel-class event timing (mvd_profile)
+  bool profiling = false;
+  std::vector<cudaEvent_t> ev_pool;
+  size_t ev_used = 0;
+  struct Rec { int cls; cudaEvent_t a, b; };
+  std::vector<Rec> recs;
+  cudaEvent_t next_event() {
+    if (ev_used == ev_pool.size()) {
+      cudaEvent_t e = nullptr;
+      if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+      ev_pool.push_back(e);
+    }
+    return ev_pool[ev_used++];
+  }
 
   float2* twx() { return reinterpret_cast<float2*>(ws + P.off_twx); }
   float2* twy() { return reinterpret_cast<float2*>(ws + P.off_twy); }
@@ -261,6 +275,24 @@ struct mvd_ctx {
 
 namespace {
 
+// brackets one launch with events while profiling is on
+struct ProfScope {
+  mvd_ctx* c;
+  cudaEvent_t a = nullptr, b = nullptr;
+  int cls;
+  ProfScope(mvd_ctx* c_, int cls_) : c(c_), cls(cls_) {
+    if (!c->profiling) return;
+    a = c->next_event();
+    b = c->next_event();
+    if (a && b) cudaEventRecord(a, c->stream);
+  }
+  ~ProfScope() {
+    if (!c->profiling || !a || !b) return;
+    cudaEventRecord(b, c->stream);
+    c->recs.push_back(mvd_ctx::Rec{cls, a, b});
+  }
+};
+
 // ---- pass launchers -------------------------------------------------------------------------
 mvd_status y_pass(mvd_ctx* c, float2* buf, int dir, int nz_planes, bool full) {
   const Plan& P = c->P;
@@ -276,7 +308,10 @@ mvd_status y_pass(mvd_ctx* c, float2* buf, int dir, int nz_planes, bool full) {
   if (full) { a.n_in = P.My; a.n_out = P.My; }
   else if (dir < 0) { a.n_in = P.N[1]; a.n_out = P.My; }
   else { a.n_in = P.My; a.n_out = P.N[1]; }
-  MVD_CK(P.ly->strided(a, dir, c->stream), "y pass");
+  {
+    ProfScope ps(c, dir < 0 ? MVD_K_Y_FWD : MVD_K_Y_INV);
+    MVD_CK(P.ly->strided(a, dir, c->stream), "y pass");
+  }
   ++c->launches;
   return MVD_OK;
 }
@@ -302,7 +337,10 @@ mvd_status z_conv(mvd_ctx* c, const float2* in, float2* out, const float2* spec)
   ZconvArgs a{};
   a.in = in; a.out = out; a.spec = spec; a.tw = c->twz();
   a.T = P.Tz; a.nthreads = P.ntz; a.plane = P.plane; a.nz = P.N[2];
-  MVD_CK(P.lz->zconv(a, c->stream), "z convolution pass");
+  {
+    ProfScope ps(c, MVD_K_Z_CONV);
+    MVD_CK(P.lz->zconv(a, c->stream), "z convolution pass");
+  }
   ++c->launches;
   return MVD_OK;
 }
@@ -323,7 +361,11 @@ XArgs x_args(mvd_ctx* c, const float2* in, float2* out, int rx) {
 }
 
 mvd_status x_pass(mvd_ctx* c, const XArgs& a, int mode) {
-  MVD_CK(c->P.lx->xrow(a, mode, c->stream), "x pass");
+  {
+    static const int cls[4] = {MVD_K_X_LOAD, MVD_K_X_QUOT, MVD_K_X_UPDATE, MVD_K_X_ACCUM};
+    ProfScope ps(c, cls[mode & 3]);
+    MVD_CK(c->P.lx->xrow(a, mode, c->stream), "x pass");
+  }
   ++c->launches;
   if (mode == X_UPDATE || (mode == X_ACCUM && (a.acc_mode == ACC_LAST || a.acc_mode == ACC_ONLY))) {
     c->stats_valid = true;
@@ -713,9 +755,38 @@ mvd_status mvd_convolve(mvd_ctx* c, int view, int which, const float* src, float
 
 long long mvd_launch_count(const mvd_ctx* c) { return c ? c->launches : 0; }
 
+mvd_status mvd_profile(mvd_ctx* c, int enable) {
+  if (!c) return MVD_ERR_INVALID_ARG;
+  if (c->broken || (enable && c->use_graph)) return MVD_ERR_STATE;
+  c->profiling = enable != 0;
+  return MVD_OK;
+}
+
+mvd_status mvd_profile_read(mvd_ctx* c, double* total_ms, long long* launches) {
+  if (!c || !total_ms || !launches) return MVD_ERR_INVALID_ARG;
+  if (c->broken) return MVD_ERR_STATE;
+  MVD_CK(cudaStreamSynchronize(c->stream), "profile read");
+  for (int k = 0; k < MVD_K_COUNT; ++k) { total_ms[k] = 0.0; launches[k] = 0; }
+  for (const mvd_ctx::Rec& r : c->recs) {
+    float ms = 0.f;
+    MVD_CK(cudaEventElapsedTime(&ms, r.a, r.b), "profile read");
+    total_ms[r.cls] += ms;
+    ++launches[r.cls];
+  }
+  c->recs.clear();
+  c->ev_used = 0;
+  return MVD_OK;
+}
+
+const char* mvd_kernel_class_name(int k) {
+  static const char* const names[MVD_K_COUNT] = {"y_fwd", "y_inv", "z_conv", "x_quot", "x_update", "x_accum", "x_load"};
+  return (k >= 0 && k < MVD_K_COUNT) ? names[k] : "";
+}
+
 void mvd_destroy(mvd_ctx* c) {
   if (!c) return;
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+  for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
   delete c;
 }
 

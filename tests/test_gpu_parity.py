@@ -1,0 +1,309 @@
+"""Parity of the CUDA path (through the C ABI, via the thin binding) with the fp64 oracle.
+
+Every test runs on the same seeded inputs on both sides (mvd_synth) and compares element by
+element.  Tolerances are the ones BASELINE.json:north_star states:
+    relative L2 <= 1e-5 after 1 iteration, <= 1e-4 after >= 10 iterations,
+    max per-voxel relative error <= 1e-3 with the denominator max(|oracle|, psi_floor)  (R12).
+The oracle side never sees a value produced by the CUDA path.
+"""
+import numpy as np
+import pytest
+
+import mvd_synth
+from oracle import mvd_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+FLOOR = 1e-6
+TOL_L2_1 = 1e-5
+TOL_L2_10 = 1e-4
+TOL_MAX = 1e-3
+
+
+def errors(g, o, floor=FLOOR):
+    g = np.asarray(g, dtype=np.float64)
+    o = np.asarray(o, dtype=np.float64)
+    rel_l2 = np.linalg.norm((g - o).ravel()) / np.linalg.norm(o.ravel())
+    rel_max = float((np.abs(g - o) / np.maximum(np.abs(o), floor)).max())
+    return float(rel_l2), rel_max
+
+
+def check(g, o, iters, what=""):
+    assert np.isfinite(g).all(), what
+    l2, mx = errors(g, o)
+    tol = TOL_L2_1 if iters <= 1 else TOL_L2_10
+    assert l2 <= tol, "%s: rel-L2 %.3g > %.1g after %d iterations" % (what, l2, tol, iters)
+    assert mx <= TOL_MAX, "%s: max per-voxel rel %.3g after %d iterations" % (what, mx, iters)
+    return l2, mx
+
+
+@pytest.fixture(scope="module")
+def mvd():
+    import torch
+    import paper_1308_0730_b200 as m
+    assert torch.cuda.is_available()
+    m.load_library()          # fails loudly if libmvd.so is missing: there is no fallback
+    return m
+
+
+def to_dev(arrs):
+    import torch
+    return [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in arrs]
+
+
+def gpu_checkpoints(mvd, prob, variant, mode, checkpoints, **kw):
+    d = mvd.Deconvolver(to_dev(prob.views), prob.psfs, variant=variant, kernel_mode=mode, **kw)
+    out, done = {}, 0
+    for c in checkpoints:
+        d.iterate(c - done)
+        done = c
+        out[c] = d.get_estimate_host()
+    stats = d.get_stats()
+    d.close()
+    return out, stats
+
+
+def oracle_checkpoints(prob, variant, mode, checkpoints, **kw):
+    o = O.Oracle(prob.views, prob.psfs, variant, kernel_mode=mode, **kw)
+    out, done = {}, 0
+    for c in checkpoints:
+        o.iterate(c - done)
+        done = c
+        out[c] = o.psi.copy()
+    return out, o
+
+
+# ------------------------------------------------------------------------------------------
+# k = 0: tiny volume, random NON-symmetric PSFs (the case a missing mirror / centre offset fails)
+# ------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def tiny():
+    return mvd_synth.make_tiny_asymmetric()
+
+
+ALL_MODES = [("independent", "auto"), ("efficient", "auto"), ("osem", "auto"), ("osem", "plain"),
+             ("efficient", "opt1"), ("osem", "opt1"), ("osem", "opt2"), ("independent", "compound")]
+
+
+@pytest.mark.parametrize("variant,mode", ALL_MODES)
+def test_tiny_asymmetric_all_variants(mvd, tiny, variant, mode):
+    g, st = gpu_checkpoints(mvd, tiny, variant, mode, (1, 3, 10))
+    o, orc = oracle_checkpoints(tiny, variant, mode, (1, 3, 10))
+    for c in (1, 3, 10):
+        check(g[c], o[c], c, "%s/%s" % (variant, mode))
+    assert st["iterations_done"] == 10
+    assert st["flux"] == pytest.approx(orc.flux, rel=1e-5)
+    assert st["l1_change"] == pytest.approx(orc.l1_change, rel=2e-3, abs=1e-3 * orc.flux * 1e-3)
+
+
+def test_tiny_direct_sum_oracle_backend(mvd, tiny):
+    """The brute-force (direct-sum) oracle, not only its FFT back-end, agrees with the GPU."""
+    small = mvd_synth.make_tiny_asymmetric(dims=(12, 10, 9), psf_dims=(5, 3, 7), n_views=2)
+    g, _ = gpu_checkpoints(mvd, small, "osem", "auto", (2,))
+    o = O.deconvolve(small.views, small.psfs, "osem", 2, backend="direct")
+    check(g[2], o, 2, "direct-sum")
+
+
+def test_tiny_literal_product(mvd, tiny):
+    """literal_product=1: the bare product of eq. 2/38/104 (R1), parity for one iteration."""
+    g, _ = gpu_checkpoints(mvd, tiny, "efficient", "auto", (1,), literal_product=True)
+    o, _ = oracle_checkpoints(tiny, "efficient", "auto", (1,), literal_product=True)
+    check(g[1], o[1], 1, "literal product")
+
+
+@pytest.mark.parametrize("mode", ["plain", "compound", "opt1", "opt2"])
+def test_back_projectors_match_oracle(mvd, tiny, mode):
+    """Device precompute of eq. 105 / 107 / 108 (fp64) against the oracle's construction."""
+    d = mvd.Deconvolver(to_dev(tiny.views), tiny.psfs, variant="osem", kernel_mode=mode)
+    psfs = [O.normalise(p) for p in tiny.psfs]
+    for v in range(tiny.n_views):
+        k = d.get_back_projector(v)
+        ref = O.back_projector(psfs, v, mode, backend="direct")
+        assert np.abs(k - ref).max() <= 1e-12 * ref.max(), (mode, v)
+    d.close()
+
+
+def test_back_projector_mixed_psf_sizes(mvd):
+    """R6: views may have PSF boxes of different sizes; factors are centre-aligned and cropped."""
+    rng = np.random.default_rng([mvd_synth.generate.SEED, 77])
+    boxes = [(5, 7, 9), (7, 5, 5), (3, 9, 7)]
+    psfs = [mvd_synth.random_psf(rng, b) for b in boxes]
+    views = [(50 * rng.random((20, 22, 26)) + 5).astype(np.float32) for _ in boxes]
+    d = mvd.Deconvolver(to_dev(views), psfs, variant="osem")
+    npsfs = [O.normalise(p) for p in psfs]
+    for v in range(3):
+        ref = O.back_projector(npsfs, v, "compound", backend="direct")
+        assert np.abs(d.get_back_projector(v) - ref).max() <= 1e-12 * ref.max()
+    d.iterate(2)
+    g = d.get_estimate_host()
+    d.close()
+    check(g, O.deconvolve(views, psfs, "osem", 2), 2, "mixed PSF boxes")
+
+
+@pytest.mark.parametrize("dims,box", [((24, 20, 18), (5, 7, 9)), ((33, 17, 9), (3, 5, 7)),
+                                      ((7, 40, 5), (7, 3, 5)), ((95, 31, 22), (9, 9, 15))])
+def test_single_convolution_matches_direct_definition(mvd, dims, box):
+    """One zero-extended 'same' convolution through the pencil-FFT path (S1/S3) against the
+    oracle, for PSF and back-projector, odd and even Nx, ragged tiles."""
+    p = mvd_synth.make_tiny_asymmetric(dims=dims, psf_dims=box, n_views=2)
+    d = mvd.Deconvolver(to_dev(p.views), p.psfs, variant="osem", kernel_mode="plain")
+    rng = np.random.default_rng(5)
+    src = rng.random(p.views[0].shape).astype(np.float32) * 10
+    import torch
+    for v in range(2):
+        pn = O.normalise(p.psfs[v])
+        for which, k in ((0, pn), (1, O.flip(pn))):
+            got = d.convolve(v, which, torch.from_numpy(src).cuda()).cpu().numpy()
+            ref = O.same_fft(src, k)
+            l2, mx = errors(got, ref)
+            assert l2 < 2e-6 and mx < 1e-4, (dims, box, v, which, l2, mx)
+    d.close()
+
+
+# ------------------------------------------------------------------------------------------
+# invariants on the GPU output itself (T4): flux identity, fixed point, identical views, delta
+# ------------------------------------------------------------------------------------------
+def test_gpu_flux_identity(mvd, tiny):
+    """P3 (eq. 52-55): plain kernel, one view-update => sum psi_new = sum phi_v."""
+    d = mvd.Deconvolver(to_dev(tiny.views[:1]), tiny.psfs[:1], variant="osem", kernel_mode="plain")
+    d.iterate(1)
+    st = d.get_stats()
+    d.close()
+    assert st["flux"] == pytest.approx(float(tiny.views[0].astype(np.float64).sum()), rel=2e-6)
+
+
+def test_gpu_fixed_point(mvd):
+    """P4 (L306): noise-free data from psi*, psi = psi* => f = same(1, K): 1 in the interior."""
+    import torch
+    p = mvd_synth.make_tiny_asymmetric(dims=(30, 28, 26), psf_dims=(5, 5, 7), n_views=2, noise=False)
+    pn = [O.normalise(q) for q in p.psfs]
+    views = [O.same_fft(p.gt, q).astype(np.float32) for q in pn]
+    d = mvd.Deconvolver(to_dev(views), p.psfs, variant="osem", kernel_mode="plain",
+                        psi0=torch.from_numpy(p.gt).cuda())
+    d.iterate(1)
+    g = d.get_estimate_host()
+    d.close()
+    # view 0 darkens the faces (R3 ii); view 1 then sees b != phi within 2r of a face and spreads
+    # that by another r: the exact fixed point survives at distance >= 3r = (9,6,6) from the faces
+    ratio = g / p.gt
+    inner = ratio[9:-9, 6:-6, 6:-6]
+    assert np.abs(inner - 1).max() < 5e-6
+    # one view alone: f = same(1, K) is 1 at distance >= r and < 1 on the faces
+    d = mvd.Deconvolver(to_dev(views[:1]), p.psfs[:1], variant="osem", kernel_mode="plain",
+                        psi0=torch.from_numpy(p.gt).cuda())
+    d.iterate(1)
+    ratio = d.get_estimate_host() / p.gt
+    d.close()
+    assert np.abs(ratio[3:-3, 2:-2, 2:-2] - 1).max() < 5e-6
+    assert ratio.min() > 0.05 and ratio.max() < 1 + 5e-6 and ratio[0, 0, 0] < 0.6
+
+
+def test_gpu_identical_views_equal_single_view(mvd, tiny):
+    """P5 (L847): V copies of one (phi, P), combined + root == one view."""
+    one, _ = gpu_checkpoints(mvd, _sub(tiny, [0]), "independent", "auto", (3,))
+    four, _ = gpu_checkpoints(mvd, _sub(tiny, [0, 0, 0, 0]), "independent", "auto", (3,))
+    l2, mx = errors(four[3], one[3])
+    assert l2 < 3e-6 and mx < 1e-4
+
+
+def test_gpu_delta_psf(mvd, tiny):
+    """P6 (L851): delta PSFs: OSEM ends on the last view, combined on the geometric mean."""
+    delta = np.zeros((3, 3, 3), np.float32)
+    delta[1, 1, 1] = 1
+    views = [v + 1 for v in tiny.views]
+    prob = mvd_synth.Problem(0, tiny.dims, (3, 3, 3), tiny.gt, [delta] * 3, views, 1, ())
+    g, _ = gpu_checkpoints(mvd, prob, "osem", "auto", (1,))
+    assert np.allclose(g[1], views[-1], rtol=3e-6)
+    g, _ = gpu_checkpoints(mvd, prob, "efficient", "auto", (1,))
+    gm = np.exp(np.mean([np.log(v.astype(np.float64)) for v in views], axis=0))
+    assert np.allclose(g[1], gm, rtol=1e-5)
+
+
+def _sub(prob, idx):
+    return mvd_synth.Problem(prob.k, prob.dims, prob.psf_dims, prob.gt, [prob.psfs[i] for i in idx],
+                             [prob.views[i] for i in idx], prob.iterations, prob.variants)
+
+
+def test_set_estimate_resume_and_graph_replay(mvd, tiny):
+    """mvd_set_estimate / psi0 resume reproduce an uninterrupted run; CUDA-graph replay of the
+    iteration gives bit-identical results to plain launches."""
+    a, _ = gpu_checkpoints(mvd, tiny, "osem", "auto", (2, 4))
+    import torch
+    d = mvd.Deconvolver(to_dev(tiny.views), tiny.psfs, variant="osem", psi0=torch.from_numpy(a[2]).cuda())
+    d.iterate(2)
+    assert np.array_equal(d.get_estimate_host(), a[4])
+    d.set_estimate(torch.from_numpy(a[2]).cuda())
+    d.iterate(2)
+    assert np.array_equal(d.get_estimate_host(), a[4])
+    d.close()
+    for variant in ("osem", "efficient"):
+        p, _ = gpu_checkpoints(mvd, tiny, variant, "auto", (3,))
+        g, _ = gpu_checkpoints(mvd, tiny, variant, "auto", (3,), use_graph=True)
+        assert np.array_equal(p[3], g[3])
+
+
+def test_eps_and_floor_clamps(mvd, tiny):
+    """R4: zero-valued data drive psi to the floor on both sides identically."""
+    views = [v.copy() for v in tiny.views]
+    for v in views:
+        v[:6] = 0
+    prob = mvd_synth.Problem(0, tiny.dims, tiny.psf_dims, tiny.gt, tiny.psfs, views, 1, ())
+    g, _ = gpu_checkpoints(mvd, prob, "osem", "auto", (12,), eps=1e-3, psi_floor=1e-2)
+    o, _ = oracle_checkpoints(prob, "osem", "auto", (12,), eps=1e-3, psi_floor=1e-2)
+    assert (o[12] == 1e-2).any()
+    assert np.isfinite(g[12]).all()
+    l2, _ = errors(g[12], o[12], 1e-2)
+    mx = float((np.abs(g[12] - o[12]) / np.maximum(np.abs(o[12]), 1e-2)).max())
+    assert l2 <= TOL_L2_10 and mx <= TOL_MAX
+
+
+# ------------------------------------------------------------------------------------------
+# BASELINE configs 1-3 at full size, every iteration count BASELINE names
+# ------------------------------------------------------------------------------------------
+def test_config1_efficient_osem_10_iterations(mvd):
+    p = mvd_synth.make_problem(1)
+    g, st = gpu_checkpoints(mvd, p, "osem", "auto", (1, 10))
+    o, orc = oracle_checkpoints(p, "osem", "auto", (1, 10))
+    check(g[1], o[1], 1, "config 1")
+    check(g[10], o[10], 10, "config 1")
+    assert st["flux"] == pytest.approx(orc.flux, rel=1e-5)
+
+
+@pytest.fixture(scope="module")
+def config2():
+    return mvd_synth.make_problem(2)
+
+
+@pytest.mark.parametrize("variant,mode", [("independent", "auto"), ("efficient", "auto"),
+                                          ("osem", "auto"), ("osem", "plain")])
+def test_config2_all_variants_20_iterations(mvd, config2, variant, mode):
+    g, _ = gpu_checkpoints(mvd, config2, variant, mode, (1, 10, 20))
+    o, _ = oracle_checkpoints(config2, variant, mode, (1, 10, 20))
+    for c in (1, 10, 20):
+        check(g[c], o[c], c, "config 2 %s/%s" % (variant, mode))
+
+
+def test_config3_efficient_osem_15_iterations(mvd):
+    p = mvd_synth.make_problem(3)
+    g, _ = gpu_checkpoints(mvd, p, "osem", "auto", (1, 15))
+    o, _ = oracle_checkpoints(p, "osem", "auto", (1, 15))
+    check(g[1], o[1], 1, "config 3")
+    check(g[15], o[15], 15, "config 3")
+
+
+# ------------------------------------------------------------------------------------------
+# block-wise mode (S6, R13)
+# ------------------------------------------------------------------------------------------
+def test_blocked_matches_blocked_oracle(mvd):
+    p = mvd_synth.make_problem(1, dims=(48, 40, 36), psf_dims=(7, 7, 11))
+    block = (20, 24, 16)                                   # (x,y,z): ragged last blocks
+    got, launches = mvd.deconvolve_blocked(to_dev(p.views), p.psfs, block, 3, variant="osem")
+    ref = O.deconvolve_blocked(p.views, p.psfs, block[::-1], "osem", 3)
+    check(got.cpu().numpy(), ref, 3, "blocked")
+    assert launches > 0
+
+
+def test_blocked_single_block_equals_whole(mvd, tiny):
+    got, _ = mvd.deconvolve_blocked(to_dev(tiny.views), tiny.psfs, (64, 64, 64), 2, variant="efficient")
+    whole, _ = gpu_checkpoints(mvd, tiny, "efficient", "auto", (2,))
+    assert np.array_equal(got.cpu().numpy(), whole[2])
