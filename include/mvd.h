@@ -24,7 +24,7 @@
  *   - Volumes are fp32, x fastest: element (x,y,z) at [(z*Ny + y)*Nx + x].  dims = {Nx,Ny,Nz}.
  *   - `views` are DEVICE pointers; they are BORROWED (read-only, never copied) and must stay valid
  *     and unchanged until mvd_destroy.
- *   - `psfs` are HOST pointers, x fastest, dims psf_dims[v] = {Kx,Ky,Kz}, all odd, K <= N per axis,
+ *   - `psfs` are HOST pointers, x fastest, dims psf_dims[v] = {Kx,Ky,Kz}, all odd (K may exceed N),
  *     values >= 0 with a positive sum (eq. 4).  They are copied during mvd_create.
  *   - ALL device memory the library uses is the caller's `workspace` (device pointer, at least
  *     mvd_workspace_size bytes, 256-byte aligned).  It must outlive the context.  The estimate psi
@@ -55,7 +55,7 @@ typedef struct mvd_ctx mvd_ctx;   /* opaque; created by mvd_create, freed by mvd
 
 typedef enum {
   MVD_OK = 0,
-  MVD_ERR_INVALID_ARG = 1,   /* NULL pointer, bad dims, even PSF size, PSF larger than volume, bad enum */
+  MVD_ERR_INVALID_ARG = 1,   /* NULL pointer, bad dims, even PSF size, bad enum */
   MVD_ERR_UNSUPPORTED = 2,   /* no FFT length available for this size */
   MVD_ERR_WORKSPACE = 3,     /* workspace NULL, misaligned or too small */
   MVD_ERR_CUDA = 4,          /* a CUDA call failed (see mvd_last_error) */
@@ -87,7 +87,7 @@ typedef struct {
   void* workspace;           /* DEVICE pointer, caller owned                                */
   size_t workspace_bytes;
   void* stream;              /* cudaStream_t                                                */
-  int use_graph;             /* 1: mvd_iterate replays one captured CUDA graph per iteration */
+  int use_graph;             /* 1: mvd_iterate replays one captured CUDA graph per iteration (needs a non-default stream: MVD_ERR_UNSUPPORTED otherwise) */
 } mvd_options;
 
 /* Fills *opt with the defaults (struct_size set, everything else 0/NULL/defaults). */

@@ -137,13 +137,15 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
   for (int v = 0; v < n_views; ++v) {
     for (int a = 0; a < 3; ++a) {
       const int k = psf_dims[v][a];
-      if (k < 1 || (k & 1) == 0 || k > dims[a]) return MVD_ERR_INVALID_ARG;
+      if (k < 1 || (k & 1) == 0 || k > (1 << 12)) return MVD_ERR_INVALID_ARG;
       P.r[a] = std::max(P.r[a], (k - 1) / 2);
     }
     P.K[v] = Dims3{psf_dims[v][0], psf_dims[v][1], psf_dims[v][2]};
   }
   P.hx = (P.N[0] + 1) / 2;
-  const int need[3] = {P.hx + 2 * P.r[0], P.N[1] + P.r[1], P.N[2] + P.r[2]};
+  // alias-free 'same' output needs M >= N + r; the wrapped kernel taps need M >= K = 2r + 1
+  const int need[3] = {P.hx + 2 * P.r[0], std::max(P.N[1] + P.r[1], 2 * P.r[1] + 1),
+                       std::max(P.N[2] + P.r[2], 2 * P.r[2] + 1)};
   const LengthOps* l[3];
   for (int a = 0; a < 3; ++a) {
     const int want = opt ? opt->fft_dims[a] : 0;
@@ -631,6 +633,11 @@ mvd_status mvd_create(mvd_ctx** out, int n_views, const float* const* views, con
   c->stream = reinterpret_cast<cudaStream_t>(opt->stream);
   c->ws = reinterpret_cast<char*>(opt->workspace);
   c->use_graph = opt->use_graph;
+  if (c->use_graph && !c->stream) {   // the legacy default stream cannot be captured
+    fprintf(stderr, "mvd_create: use_graph needs a non-default stream\n");
+    delete c;
+    return MVD_ERR_UNSUPPORTED;
+  }
   c->views.assign(views, views + n_views);
 
   cudaError_t e = cudaSuccess;
