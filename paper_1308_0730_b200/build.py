@@ -49,7 +49,7 @@ def _run(cmd):
 
 def build(jobs=None, force=False, verbose=True):
     os.makedirs(OBJ, exist_ok=True)
-    hdr = [os.path.join(CSRC, f) for f in ("fft_reg.cuh", "pass_kernels.cuh", "fft_ops.h")]
+    hdr = [os.path.join(CSRC, f) for f in ("fft_reg.cuh", "pass_kernels.cuh", "pass_tma.cuh", "async_copy.cuh", "fft_ops.h")]
     tasks = []
     objs = []
     for a, b in lengths():
@@ -58,7 +58,7 @@ def build(jobs=None, force=False, verbose=True):
         src = os.path.join(CSRC, "inst.cu")
         if force or _newer(o, hdr + [src]):
             tasks.append([NVCC, *FLAGS, "-DMVD_INST_A=%d" % a, "-DMVD_INST_B=%d" % b, "-c", src, "-o", o])
-    host_deps = hdr[2:] + [os.path.join(CSRC, f) for f in ("mvd.cu", "misc_kernels.cuh", "lengths.def")] + \
+    host_deps = hdr[4:] + [os.path.join(CSRC, f) for f in ("mvd.cu", "misc_kernels.cuh", "lengths.def")] + \
         [os.path.join(os.path.dirname(HERE), "include", "mvd.h")]
     for name in ("mvd",):
         o = os.path.join(OBJ, name + ".o")

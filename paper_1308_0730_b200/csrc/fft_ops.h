@@ -65,6 +65,10 @@ struct XArgs {
   int acc_mode;            // AccMode
   int literal_product;
   int complex_in;          // X_LOAD: rows of `in` are complex and transformed in full
+  // TMA-staged variant (pass_tma.cuh)
+  int real_stride;         // floats between real rows in shared memory
+  int bulk_real;           // real rows are 16-byte aligned: staged by bulk copies (else plain loads)
+  int grid;                // persistent CTAs
 };
 
 struct LengthOps {
@@ -76,6 +80,10 @@ struct LengthOps {
   cudaError_t (*xrow)(const XArgs&, int mode, cudaStream_t);
   size_t (*strided_smem)(int T);
   size_t (*xrow_smem)(int rows, int rx);
+  // TMA-staged passes (pass_tma.cuh)
+  cudaError_t (*xrow_tma)(const XArgs&, int mode, cudaStream_t);
+  size_t (*xrow_tma_smem)(int rows, int rx, int nx);
+  int (*xrow_tma_blocks_per_sm)(int mode, int nthreads, size_t smem);
 };
 
 // table of all compiled lengths, ascending in M

@@ -1,6 +1,6 @@
 // One translation unit per supported pencil length: compiled once for every MVD_LEN(A, B) line of
 // lengths.def with -DMVD_INST_A=A -DMVD_INST_B=B (see ../build.py).
-#include "pass_kernels.cuh"
+#include "pass_tma.cuh"
 
 #if !defined(MVD_INST_A) || !defined(MVD_INST_B)
 #error "compile with -DMVD_INST_A=<A> -DMVD_INST_B=<B>"
@@ -11,5 +11,15 @@
 
 namespace mvd {
 extern const LengthOps MVD_CAT(ops_, MVD_INST_A, _, MVD_INST_B);
-const LengthOps MVD_CAT(ops_, MVD_INST_A, _, MVD_INST_B) = Launch<MVD_INST_A, MVD_INST_B>::ops();
+namespace {
+using L = Launch<MVD_INST_A, MVD_INST_B>;
+using LT = LaunchTma<MVD_INST_A, MVD_INST_B>;
+cudaError_t init_all() {
+  cudaError_t e = L::init();
+  return e != cudaSuccess ? e : LT::init();
+}
+}  // namespace
+const LengthOps MVD_CAT(ops_, MVD_INST_A, _, MVD_INST_B) = {
+    L::Cfg::M, MVD_INST_A, MVD_INST_B, L::Cfg::MAX_THREADS, &init_all, &L::strided, &L::zconv, &L::xrow,
+    &L::strided_smem, &L::xrow_smem, &LT::xrow, &LT::xrow_smem, &LT::xrow_blocks_per_sm};
 }  // namespace mvd

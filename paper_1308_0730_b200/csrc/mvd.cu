@@ -48,10 +48,13 @@ const LengthOps* const* length_table(int* count) {
   return sorted.data();
 }
 
-static const LengthOps* find_length(int min_len, int exact) {
+// smallest compiled length >= min_len (or exactly `exact`); need_even: the x length, whose rows are
+// staged by 16-byte bulk copies and whose pitch is a TMA stride
+static const LengthOps* find_length(int min_len, int exact, bool need_even) {
   int n;
   const LengthOps* const* t = length_table(&n);
   for (int i = 0; i < n; ++i) {
+    if (need_even && (t[i]->M & 1)) continue;
     if (exact > 0) {
       if (t[i]->M == exact) return t[i]->M >= min_len ? t[i] : nullptr;
     } else if (t[i]->M >= min_len) {
@@ -81,6 +84,8 @@ struct Plan {
   // tiles
   int Ty = 0, nty = 0, Tz = 0, ntz = 0, Tzs = 0, ntzs = 0, Tys = 0, ntys = 0, Rx = 0, ntx = 0;
   int nctax = 0;
+  // TMA-staged x pass
+  int xtma = 0, Rxt = 0, ntxt = 0, xt_rstride = 0;
   // workspace offsets (bytes)
   size_t off_twx = 0, off_twy = 0, off_twz = 0, off_psi = 0, off_acc = 0, off_w = 0, off_w0 = 0,
          off_spec = 0, off_psf = 0, off_kern = 0, off_auto = 0, off_stage = 0, off_partials = 0,
@@ -150,7 +155,7 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
   for (int a = 0; a < 3; ++a) {
     const int want = opt ? opt->fft_dims[a] : 0;
     if (want < 0) return MVD_ERR_INVALID_ARG;
-    l[a] = find_length(need[a], want);
+    l[a] = find_length(need[a], want, a == 0);
     if (!l[a]) return want > 0 ? MVD_ERR_INVALID_ARG : MVD_ERR_UNSUPPORTED;
   }
   P.lx = l[0]; P.ly = l[1]; P.lz = l[2];
@@ -176,6 +181,24 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
     // spectrum construction runs the same kernel over My*Mz rows
     const long long rows_max = std::max((long long)P.N[1] * P.N[2], (long long)P.My * P.Mz);
     P.nctax = (int)((rows_max + R - 1) / R);
+  }
+
+  {
+    // TMA-staged x pass (quotient / OSEM update): rows per tile sized for >= 3 resident CTAs per SM
+    const int ab = std::max(P.lx->A, P.lx->B);
+    P.xtma = env_int("MVD_XTMA", 1);
+    int R = std::max(1, 256 / ab);
+    const int force = env_int("MVD_RXT", 0);
+    const size_t cap = (size_t)env_int("MVD_XT_SMEM_KB", 72) * 1024;
+    while (R > 1 && P.lx->xrow_tma_smem(R, P.r[0], P.N[0]) > cap) --R;
+    if (force > 0 && force * ab <= 256 && P.lx->xrow_tma_smem(force, P.r[0], P.N[0]) <= 220 * 1024) R = force;
+    if (P.lx->xrow_tma_smem(R, P.r[0], P.N[0]) > 220 * 1024) P.xtma = 0;
+    P.Rxt = R;
+    P.ntxt = round_up32(R * ab);
+    int s = (P.N[0] + 3) / 4 * 4;
+    const int want = (P.lx->B % 32) / 4 * 4;
+    while ((s % 32) != want) s += 4;
+    P.xt_rstride = s;
   }
 
   // workspace layout
@@ -233,6 +256,8 @@ struct mvd_ctx {
   cudaGraphExec_t graph_exec = nullptr;
   long long graph_launches = 0;
   char err[512] = {0};
+  int num_sms = 148;
+  int xt_blocks[4] = {0, 0, 0, 0};   // resident CTAs per SM of the TMA-staged x pass, per mode
   // per-kernel-class event timing (mvd_profile)
   bool profiling = false;
   std::vector<cudaEvent_t> ev_pool;
@@ -362,16 +387,36 @@ XArgs x_args(mvd_ctx* c, const float2* in, float2* out, int rx) {
   return a;
 }
 
-mvd_status x_pass(mvd_ctx* c, const XArgs& a, int mode) {
-  {
-    static const int cls[4] = {MVD_K_X_LOAD, MVD_K_X_QUOT, MVD_K_X_UPDATE, MVD_K_X_ACCUM};
+mvd_status x_pass(mvd_ctx* c, const XArgs& a_in, int mode) {
+  static const int cls[4] = {MVD_K_X_LOAD, MVD_K_X_QUOT, MVD_K_X_UPDATE, MVD_K_X_ACCUM};
+  const Plan& P = c->P;
+  XArgs a = a_in;
+  const bool tma = P.xtma && (mode == X_QUOT || mode == X_UPDATE);
+  if (tma) {
+    // persistent CTAs, tiles of Rxt rows staged by bulk copies (pass_tma.cuh)
+    a.rows_per_cta = P.Rxt;
+    a.nthreads = P.ntxt;
+    a.real_stride = P.xt_rstride;
+    const float* real_src = mode == X_QUOT ? a.phi : a.psi;
+    a.bulk_real = (P.N[0] % 4 == 0) && ((reinterpret_cast<size_t>(real_src) & 15) == 0);
+    if (c->xt_blocks[mode] == 0) {
+      c->xt_blocks[mode] = P.lx->xrow_tma_blocks_per_sm(mode, a.nthreads, P.lx->xrow_tma_smem(a.rows_per_cta, P.r[0], P.N[0]));
+      if (c->xt_blocks[mode] <= 0) { snprintf(c->err, sizeof(c->err), "x pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
+    }
+    const long long ntiles = (a.nrows + a.rows_per_cta - 1) / a.rows_per_cta;
+    a.grid = (int)std::min<long long>(std::min<long long>(ntiles, (long long)c->num_sms * c->xt_blocks[mode]), P.sum_blocks);
+    {
+      ProfScope ps(c, cls[mode & 3]);
+      MVD_CK(P.lx->xrow_tma(a, mode, c->stream), "x pass (TMA)");
+    }
+  } else {
     ProfScope ps(c, cls[mode & 3]);
-    MVD_CK(c->P.lx->xrow(a, mode, c->stream), "x pass");
+    MVD_CK(P.lx->xrow(a, mode, c->stream), "x pass");
   }
   ++c->launches;
   if (mode == X_UPDATE || (mode == X_ACCUM && (a.acc_mode == ACC_LAST || a.acc_mode == ACC_ONLY))) {
     c->stats_valid = true;
-    c->stats_ncta = (int)((a.nrows + a.rows_per_cta - 1) / a.rows_per_cta);
+    c->stats_ncta = tma ? a.grid : (int)((a.nrows + a.rows_per_cta - 1) / a.rows_per_cta);
   }
   return MVD_OK;
 }
@@ -641,10 +686,18 @@ mvd_status mvd_create(mvd_ctx** out, int n_views, const float* const* views, con
   c->views.assign(views, views + n_views);
 
   cudaError_t e = cudaSuccess;
+  {
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+  }
   const LengthOps* ls[3] = {c->P.lx, c->P.ly, c->P.lz};
   for (int a = 0; a < 3 && e == cudaSuccess; ++a) e = ls[a]->init();
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-  if (e != cudaSuccess) { delete c; return MVD_ERR_CUDA; }
+  if (e != cudaSuccess) {
+    fprintf(stderr, "mvd_create: kernel attribute setup failed: %s\n", cudaGetErrorString(e));
+    delete c;
+    return MVD_ERR_CUDA;
+  }
 
   s = precompute(c, psfs);
   if (s == MVD_OK) s = init_estimate(c, opt->psi0);

@@ -478,10 +478,6 @@ struct Launch {
     return cudaGetLastError();
   }
 
-  static constexpr LengthOps ops() {
-    return LengthOps{Cfg::M, A, B, Cfg::MAX_THREADS, &init, &strided, &zconv, &xrow,
-                     &strided_smem, &xrow_smem};
-  }
 };
 
 }  // namespace mvd

@@ -1,0 +1,296 @@
+// TMA-staged pencil passes (sm_100a): the same transforms as pass_kernels.cuh, with every HBM
+// read staged through shared memory by the copy engine (async_copy.cuh), persistent CTAs and
+// double-buffered tiles, so the next tile is in flight while the current one is transformed and
+// no load ever sits in registers or L1.
+//
+//   xrow_tma_kernel   : x-inverse -> crop + quotient / OSEM update -> zero-pad + x-forward
+//                       (S2 / S4 of DESIGN.md; eq. 13, eq. 109-112)
+//   strided_tma_kernel: y pass, form F, pruned input (TMA zero fill) / cropped output
+//   zconv_tma_kernel  : z-forward . spectrum . z-inverse, input tile and spectrum tile by TMA
+#pragma once
+
+#include <cstdio>
+
+#include "async_copy.cuh"
+#include "pass_kernels.cuh"
+
+namespace mvd {
+
+// shared-memory row strides of the x pass that keep the column accesses conflict-free
+//   complex rows: stride == A or A+1 (mod 16) float2 and even (16-byte rows for the bulk copy)
+//   real rows   : stride a multiple of 4 floats, as close to B (mod 32) as that allows
+__host__ __device__ constexpr int xrow_cstride(int M, int A) {
+  int s = M;
+  while ((s & 1) || !((s % 16) == (A % 16) || (s % 16) == ((A + 1) % 16))) ++s;
+  return s;
+}
+__host__ __device__ constexpr int xrow_rstride(int nx, int B) {
+  int s = (nx + 3) / 4 * 4;
+  const int want = (B % 32) / 4 * 4;
+  while ((s % 32) != want) s += 4;
+  return s;
+}
+
+template <int A, int B, int MODE>
+__global__ void __launch_bounds__(256) xrow_tma_kernel(const XArgs p) {
+  using Cfg = PassCfg<A, B>;
+  constexpr int M = Cfg::M, AP = Cfg::AP, BP = Cfg::BP, RS = Cfg::ROW_F2;
+  constexpr int CS = xrow_cstride(M, A);
+  static_assert(MODE == X_QUOT || MODE == X_UPDATE, "TMA-staged x pass: quotient and OSEM update only");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int R = p.rows_per_cta;
+  const int RSTR = p.real_stride;
+  // layout: [2 stages][R][CS] float2 | [2 stages][R][RSTR] float | exch [R][RS] float2 | halos | barriers
+  float2* wst = reinterpret_cast<float2*>(smem_raw);
+  float* rst = reinterpret_cast<float*>(wst + (size_t)2 * R * CS);
+  float2* sm = reinterpret_cast<float2*>(rst + (size_t)2 * R * RSTR);
+  float* halo_re = reinterpret_cast<float*>(sm + (size_t)R * RS);
+  float* halo_im = halo_re + R * p.rx;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(
+      (reinterpret_cast<uintptr_t>(halo_im + R * p.rx) + 7) & ~uintptr_t(7));
+  const int tid = threadIdx.x;
+  const float* real_src = MODE == X_QUOT ? p.phi : p.psi;
+  const int ntiles = (int)((p.nrows + R - 1) / R);
+
+  if (tid == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  // warp 0 issues the copies of a tile: lane l stages complex and real rows l, l+32, ...
+  const int nrows_i = (int)p.nrows;
+  auto issue = [&](int tile, int s) {
+    const int row0 = tile * R;
+    const int rv = min(R, nrows_i - row0);
+    if (tid == 0)
+      mbar_expect_tx(&bars[s], (uint32_t)rv * (uint32_t)(M * sizeof(float2) + (p.bulk_real ? p.nx * sizeof(float) : 0)));
+    __syncwarp();
+    for (int r = tid; r < rv; r += 32) {
+      const unsigned g = (unsigned)(row0 + r);
+      const unsigned zq = g / (unsigned)p.ny_rows, yr = g - zq * (unsigned)p.ny_rows;
+      const long long off = (long long)zq * p.plane_pitch + (long long)yr * M;
+      bulk_g2s(wst + ((size_t)s * R + r) * CS, p.in + off, M * sizeof(float2), &bars[s]);
+      if (p.bulk_real)
+        bulk_g2s(rst + ((size_t)s * R + r) * RSTR, real_src + (long long)g * p.nx, p.nx * sizeof(float), &bars[s]);
+    }
+  };
+
+  const int rowA = tid / A, k1 = tid - rowA * A;
+  const int rowB = tid / B, n2 = tid - rowB * B;
+  double dflux = 0.0, dl1 = 0.0;
+
+  if (tid < 32 && (int)blockIdx.x < ntiles) issue((int)blockIdx.x, 0);
+
+  int it = 0;
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+    const int s = it & 1;
+    const int row0 = tile * R;
+    const int growA = row0 + rowA, growB = row0 + rowB;
+    const bool actA = tid < R * A && growA < nrows_i;
+    const bool actB = tid < R * B && growB < nrows_i;
+    // stage s^1 was last read before the barriers of the previous tile: refill it now
+    if (tid < 32 && tile + (int)gridDim.x < ntiles) issue(tile + (int)gridDim.x, s ^ 1);
+    if (!p.bulk_real) {   // rows not 16-byte aligned: plain loads of this tile's real rows
+      const int rv = min(R, nrows_i - row0);
+      for (int i = tid; i < rv * p.nx; i += blockDim.x) {
+        const int r = i / p.nx, x = i - r * p.nx;
+        rst[((size_t)s * R + r) * RSTR + x] = real_src[(long long)(row0 + r) * p.nx + x];
+      }
+      __syncthreads();
+    }
+    mbar_wait(&bars[s], (it >> 1) & 1);
+
+    float2 c[A];
+    float flux = 0.f, l1 = 0.f;
+    // ---- G1: inverse B-point transforms over k2 ------------------------------------------------
+    if (actA) {
+      float2 u[B];
+      const float2* src = wst + ((size_t)s * R + rowA) * CS + k1;
+      static_for<0, B>([&](auto k2_) {
+        constexpr int k2 = decltype(k2_)::value;
+        u[k2] = src[A * k2];
+      });
+      FftReg<B, 1>::run(u);
+      float2 pw[B];
+      const float2 w = ld_tw(p.tw, k1);
+      powers<B>(make_float2(w.x, -w.y), pw);
+      static_for<0, B>([&](auto n2_) {
+        constexpr int m = decltype(n2_)::value;
+        if constexpr (m > 0) u[m] = cmul(u[m], pw[m]);
+        sm[rowA * RS + m * AP + k1] = u[m];
+      });
+    }
+    __syncthreads();
+    // ---- G2: inverse A-point transforms over k1 -> c[n1], n = n1*B + n2 ------------------------
+    if (actB) {
+      static_for<0, A>([&](auto k1_) {
+        constexpr int kk = decltype(k1_)::value;
+        c[kk] = sm[rowB * RS + n2 * AP + kk];
+      });
+      FftReg<A, 1>::run(c);
+      static_for<0, A>([&](auto n1_) {
+        constexpr int n1 = decltype(n1_)::value;
+        // warp-uniform: does [n1*B, n1*B + B) touch an overlap region at all?
+        if (n1 * B + B > p.hx && (n1 * B < p.hx + p.rx || n1 * B + B > M - p.rx)) {
+          const int n = n1 * B + n2;
+          if (n >= p.hx && n < p.hx + p.rx) halo_re[rowB * p.rx + (n - p.hx)] = c[n1].x;
+          if (n >= M - p.rx) halo_im[rowB * p.rx + (n - (M - p.rx))] = c[n1].y;
+        }
+      });
+    }
+    __syncthreads();
+    // ---- pointwise stage on the real row -------------------------------------------------------
+    if (actB) {
+      const long long rbase = (long long)growB * p.nx;
+      const float* rrow = rst + ((size_t)s * R + rowB) * RSTR;
+      float* prow = p.psi + rbase;
+      const int lo_int = p.rx, hi_int = min(p.hx - p.rx, p.nx - p.hx);   // interior: no overlap, both halves live
+      static_for<0, A>([&](auto n1_) {
+        constexpr int n1 = decltype(n1_)::value;
+        const int n = n1 * B + n2;
+        float2 z = make_float2(0.f, 0.f);
+        if (n1 * B >= lo_int && n1 * B + B <= hi_int) {     // warp-uniform fast path
+          if constexpr (MODE == X_QUOT) {
+            z.x = __fdividef(rrow[n], fmaxf(c[n1].x, p.eps));
+            z.y = __fdividef(rrow[n + p.hx], fmaxf(c[n1].y, p.eps));
+          } else {
+            const float o = rrow[n], o2 = rrow[n + p.hx];
+            const float nw = fmaxf(o * c[n1].x, p.psi_floor), nw2 = fmaxf(o2 * c[n1].y, p.psi_floor);
+            prow[n] = nw;
+            prow[n + p.hx] = nw2;
+            flux += nw + nw2;
+            l1 += fabsf(nw - o) + fabsf(nw2 - o2);
+            z = make_float2(nw, nw2);
+          }
+        } else if (n < p.hx) {
+          float vt = c[n1].x, vb = c[n1].y;
+          if (n >= p.hx - p.rx) vt += halo_im[rowB * p.rx + (n - (p.hx - p.rx))];
+          if (n < p.rx) vb += halo_re[rowB * p.rx + n];
+          const bool has_b = n + p.hx < p.nx;
+          if constexpr (MODE == X_QUOT) {
+            z.x = __fdividef(rrow[n], fmaxf(vt, p.eps));
+            if (has_b) z.y = __fdividef(rrow[n + p.hx], fmaxf(vb, p.eps));
+          } else {
+            const float o = rrow[n];
+            const float nw = fmaxf(o * vt, p.psi_floor);
+            p.psi[rbase + n] = nw;
+            flux += nw;
+            l1 += fabsf(nw - o);
+            z.x = nw;
+            if (has_b) {
+              const float o2 = rrow[n + p.hx];
+              const float nw2 = fmaxf(o2 * vb, p.psi_floor);
+              p.psi[rbase + n + p.hx] = nw2;
+              flux += nw2;
+              l1 += fabsf(nw2 - o2);
+              z.y = nw2;
+            }
+          }
+        }
+        c[n1] = z;
+      });
+      // ---- F1: forward A-point transforms over n1 ----------------------------------------------
+      FftReg<A, -1>::run(c);
+      float2 pw[A];
+      powers<A>(ld_tw(p.tw, n2), pw);
+      static_for<0, A>([&](auto k1_) {
+        constexpr int kk = decltype(k1_)::value;
+        if constexpr (kk > 0) c[kk] = cmul(c[kk], pw[kk]);
+        sm[rowB * RS + kk * BP + n2] = c[kk];
+      });
+    }
+    __syncthreads();
+    // ---- F2: forward B-point transforms over n2, store k = k1 + A*k2 ---------------------------
+    if (actA) {
+      float2 u[B];
+      static_for<0, B>([&](auto n2_) {
+        constexpr int m = decltype(n2_)::value;
+        u[m] = sm[rowA * RS + k1 * BP + m];
+      });
+      FftReg<B, -1>::run(u);
+      const unsigned zq = (unsigned)growA / (unsigned)p.ny_rows, yr = (unsigned)growA - zq * (unsigned)p.ny_rows;
+      float2* dst = p.out + (long long)zq * p.plane_pitch + (long long)yr * M + k1;
+      static_for<0, B>([&](auto k2_) {
+        constexpr int k2 = decltype(k2_)::value;
+        dst[A * k2] = u[k2];
+      });
+    }
+    dflux += (double)flux;
+    dl1 += (double)l1;
+    __syncthreads();   // the exchange buffer is rewritten by the next tile's G1
+  }
+
+  // ---- per-CTA statistics of the update: {sum psi_new, sum |psi_new - psi_old|} ----------------
+  if constexpr (MODE == X_UPDATE) {
+    double df = dflux, dl = dl1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      df += __shfl_down_sync(0xffffffffu, df, o);
+      dl += __shfl_down_sync(0xffffffffu, dl, o);
+    }
+    __shared__ double red[2][32];
+    const int warp = tid >> 5, lane = tid & 31;
+    if (lane == 0) { red[0][warp] = df; red[1][warp] = dl; }
+    __syncthreads();
+    if (warp == 0) {
+      const int nw = (blockDim.x + 31) >> 5;
+      df = lane < nw ? red[0][lane] : 0.0;
+      dl = lane < nw ? red[1][lane] : 0.0;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        df += __shfl_down_sync(0xffffffffu, df, o);
+        dl += __shfl_down_sync(0xffffffffu, dl, o);
+      }
+      if (lane == 0) {
+        p.partials[2 * (size_t)blockIdx.x] = df;
+        p.partials[2 * (size_t)blockIdx.x + 1] = dl;
+      }
+    }
+  }
+}
+
+// host-side launchers of the TMA-staged passes
+template <int A, int B>
+struct LaunchTma {
+  using Cfg = PassCfg<A, B>;
+
+  static size_t xrow_smem(int rows, int rx, int nx) {
+    return (size_t)2 * rows * xrow_cstride(Cfg::M, A) * sizeof(float2) +
+           (size_t)2 * rows * xrow_rstride(nx, B) * sizeof(float) + (size_t)rows * Cfg::ROW_F2 * sizeof(float2) +
+           (size_t)2 * rows * rx * sizeof(float) + 32;
+  }
+
+  static cudaError_t init() {
+    cudaError_t e;
+#define MVD_SET(k) \
+  e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024); \
+  if (e != cudaSuccess) { fprintf(stderr, "smem attr failed %d x %d: %s\n", A, B, #k); return e; } \
+  e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \
+  if (e != cudaSuccess) { fprintf(stderr, "carveout attr failed %d x %d: %s\n", A, B, #k); return e; }
+    MVD_SET((xrow_tma_kernel<A, B, X_QUOT>));
+    MVD_SET((xrow_tma_kernel<A, B, X_UPDATE>));
+#undef MVD_SET
+    return cudaSuccess;
+  }
+
+  static int xrow_blocks_per_sm(int mode, int nthreads, size_t smem) {
+    int n = 0;
+    cudaError_t e = mode == X_QUOT
+        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_QUOT>, nthreads, smem)
+        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_UPDATE>, nthreads, smem);
+    return e == cudaSuccess ? n : 0;
+  }
+
+  static cudaError_t xrow(const XArgs& a, int mode, cudaStream_t s) {
+    if (a.grid <= 0) return cudaSuccess;
+    const size_t smem = xrow_smem(a.rows_per_cta, a.rx, a.nx);
+    if (mode == X_QUOT) xrow_tma_kernel<A, B, X_QUOT><<<a.grid, a.nthreads, smem, s>>>(a);
+    else if (mode == X_UPDATE) xrow_tma_kernel<A, B, X_UPDATE><<<a.grid, a.nthreads, smem, s>>>(a);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
+  }
+};
+
+}  // namespace mvd
