@@ -3,9 +3,39 @@
 // instantiated once per length in inst.cu; mvd.cu only sees this table.
 #pragma once
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 namespace mvd {
+
+// ---- TMA-staged strided pass (pass_tma.cuh): persistent CTAs, tiles of T contiguous complex
+//      elements x the whole pencil, loaded by tensor copies with zero fill beyond n_in ----------
+struct StridedTmaArgs {
+  CUtensorMap in_map;      // dims (x: line_len, pencil: n_in, outer: n_outer); box (T, boxr, 1)
+  float2* out;
+  const float2* tw;        // tw[j] = exp(-2*pi*i*j/M)
+  int T, nthreads, grid;
+  int boxr, nbox;          // the pencil is staged as nbox boxes of boxr rows (boxr*nbox >= M)
+  int xt0, n_xt;           // x tiles [xt0, xt0 + n_xt) of every line are processed
+  int line_len;            // contiguous extent (complex elements)
+  int n_outer;
+  long long out_outer_stride, out_pstride;
+  int n_out;               // pencil outputs >= n_out are not stored
+};
+
+// ---- TMA-staged fused z pass: input tile and spectrum tile by tensor copies --------------------
+struct ZconvTmaArgs {
+  CUtensorMap in_map;      // dims (x: Mx, y: My, z: nz);  box (T, 1, boxr)
+  CUtensorMap spec_map;    // dims (x: Mx, y: My, z: Mz);  box (T, 1, boxr)
+  float2* out;
+  const float2* tw;
+  int T, nthreads, grid;
+  int boxr, nbox;
+  int xt0, n_xt;           // x tiles [xt0, xt0 + n_xt) of every row
+  int mx, my;              // row length and rows per plane
+  long long plane;         // elements between z planes of `out`
+  int nz;                  // planes written
+};
 
 // ---- strided pencil FFT (y pass, plain z pass): pencils along a strided axis, tiles of T
 //      contiguous complex elements across the unit-stride axis --------------------------------
@@ -84,6 +114,12 @@ struct LengthOps {
   cudaError_t (*xrow_tma)(const XArgs&, int mode, cudaStream_t);
   size_t (*xrow_tma_smem)(int rows, int rx, int nx);
   int (*xrow_tma_blocks_per_sm)(int mode, int nthreads, size_t smem);
+  cudaError_t (*strided_tma)(const StridedTmaArgs&, int dir, cudaStream_t);
+  size_t (*strided_tma_smem)(int T, int boxr, int nbox);
+  int (*strided_tma_blocks_per_sm)(int dir, int nthreads, size_t smem);
+  cudaError_t (*zconv_tma)(const ZconvTmaArgs&, cudaStream_t);
+  size_t (*zconv_tma_smem)(int T, int boxr, int nbox);
+  int (*zconv_tma_blocks_per_sm)(int nthreads, size_t smem);
 };
 
 // table of all compiled lengths, ascending in M

@@ -86,6 +86,9 @@ struct Plan {
   int nctax = 0;
   // TMA-staged x pass
   int xtma = 0, Rxt = 0, ntxt = 0, xt_rstride = 0;
+  // TMA-staged y and z passes: tile width, threads, pencil boxes (boxr rows x nbox >= M)
+  int ytma = 0, Tyt = 0, ntyt = 0, ybox = 0, ynbox = 0;
+  int ztma = 0, Tzt = 0, ntzt = 0, zbox = 0, znbox = 0;
   // workspace offsets (bytes)
   size_t off_twx = 0, off_twy = 0, off_twz = 0, off_psi = 0, off_acc = 0, off_w = 0, off_w0 = 0,
          off_spec = 0, off_psf = 0, off_kern = 0, off_auto = 0, off_stage = 0, off_partials = 0,
@@ -184,6 +187,39 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
   }
 
   {
+    // TMA-staged y and z passes: tile widths are multiples of 4 (16-byte rows, 128-byte boxes)
+    auto plan_tma = [&](const LengthOps* l, int L, int force, size_t smem_cap, bool zconv, int* T_out,
+                        int* nt_out, int* box_out, int* nbox_out) {
+      const int ab = std::max(l->A, l->B);
+      const int nbox = (l->M + 255) / 256;
+      const int boxr = ((l->M + nbox - 1) / nbox + 3) / 4 * 4;
+      int best = 0;
+      double best_score = -1.0;
+      const int cand[] = {8, 12, 16, 20, 24, 4};
+      for (int T : cand) {
+        const size_t smem = zconv ? l->zconv_tma_smem(T, boxr, nbox) : l->strided_tma_smem(T, boxr, nbox);
+        if (smem > smem_cap && T > 4) continue;
+        const double eff = double(L) / double(((L + T - 1) / T) * T);
+        const double seg = T >= 8 ? 1.0 : 0.7;
+        if (eff * seg > best_score + 1e-9) { best_score = eff * seg; best = T; }
+      }
+      if (best == 0) best = 4;
+      if (force > 0 && force % 4 == 0) best = force;
+      const int items = best * ab;
+      const int rounds = (items + l->max_threads - 1) / l->max_threads;
+      *T_out = best;
+      *nt_out = std::min(l->max_threads, round_up32((items + rounds - 1) / rounds));
+      *box_out = boxr;
+      *nbox_out = nbox;
+      const size_t smem = zconv ? l->zconv_tma_smem(best, boxr, nbox) : l->strided_tma_smem(best, boxr, nbox);
+      return smem <= 220 * 1024;
+    };
+    P.ytma = env_int("MVD_YTMA", 1);
+    P.ztma = env_int("MVD_ZTMA", 1);
+    if (!plan_tma(P.ly, P.Mx, env_int("MVD_TYT", 0), (size_t)env_int("MVD_YT_SMEM_KB", 72) * 1024, false, &P.Tyt, &P.ntyt, &P.ybox, &P.ynbox)) P.ytma = 0;
+    if (!plan_tma(P.lz, P.Mx, env_int("MVD_TZT", 0), (size_t)env_int("MVD_ZT_SMEM_KB", 110) * 1024, true, &P.Tzt, &P.ntzt, &P.zbox, &P.znbox)) P.ztma = 0;
+  }
+  {
     // TMA-staged x pass (quotient / OSEM update): rows per tile sized for >= 3 resident CTAs per SM
     const int ab = std::max(P.lx->A, P.lx->B);
     P.xtma = env_int("MVD_XTMA", 1);
@@ -258,6 +294,8 @@ struct mvd_ctx {
   char err[512] = {0};
   int num_sms = 148;
   int xt_blocks[4] = {0, 0, 0, 0};   // resident CTAs per SM of the TMA-staged x pass, per mode
+  int yt_blocks[2] = {0, 0};         // ... of the TMA-staged y pass (forward, inverse)
+  int zt_blocks = 0;                 // ... of the TMA-staged z pass
   // per-kernel-class event timing (mvd_profile)
   bool profiling = false;
   std::vector<cudaEvent_t> ev_pool;
@@ -320,9 +358,93 @@ struct ProfScope {
   }
 };
 
+// ---- tensor maps (driver entry point resolved through the runtime: no link against libcuda) --
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+// 3-D map over complex64 elements (carried as 8-byte words): dims d0 (contiguous), d1, d2 with
+// element strides s1, s2; box b0 x b1 x b2; elements outside the dims are delivered as zeros
+bool make_map3(CUtensorMap* m, const void* base, long long d0, long long d1, long long d2, long long s1,
+               long long s2, int b0, int b1, int b2) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) return false;
+  const cuuint64_t gdim[3] = {(cuuint64_t)d0, (cuuint64_t)d1, (cuuint64_t)d2};
+  const cuuint64_t gstr[2] = {(cuuint64_t)s1 * 8, (cuuint64_t)s2 * 8};
+  const cuuint32_t box[3] = {(cuuint32_t)b0, (cuuint32_t)b1, (cuuint32_t)b2};
+  const cuuint32_t est[3] = {1, 1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT64, 3, const_cast<void*>(base), gdim, gstr, box, est,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+mvd_status y_pass_tma(mvd_ctx* c, float2* buf, int dir, int nz_planes, int xt0, int n_xt) {
+  const Plan& P = c->P;
+  StridedTmaArgs a{};
+  const int n_in = dir < 0 ? P.N[1] : P.My;
+  if (!make_map3(&a.in_map, buf, P.Mx, n_in, nz_planes, P.Mx, P.plane, P.Tyt, P.ybox, 1)) {
+    snprintf(c->err, sizeof(c->err), "y pass: cuTensorMapEncodeTiled failed");
+    c->broken = true;
+    return MVD_ERR_CUDA;
+  }
+  a.out = buf; a.tw = c->twy();
+  a.T = P.Tyt; a.nthreads = P.ntyt; a.boxr = P.ybox; a.nbox = P.ynbox;
+  a.xt0 = xt0; a.n_xt = n_xt;
+  a.line_len = P.Mx; a.n_outer = nz_planes;
+  a.out_outer_stride = P.plane; a.out_pstride = P.Mx;
+  a.n_out = dir < 0 ? P.My : P.N[1];
+  int& bl = c->yt_blocks[dir < 0 ? 0 : 1];
+  if (bl == 0) bl = P.ly->strided_tma_blocks_per_sm(dir, a.nthreads, P.ly->strided_tma_smem(a.T, a.boxr, a.nbox));
+  if (bl <= 0) { snprintf(c->err, sizeof(c->err), "y pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
+  a.grid = (int)std::min<long long>((long long)n_xt * nz_planes, (long long)c->num_sms * bl);
+  {
+    ProfScope ps(c, dir < 0 ? MVD_K_Y_FWD : MVD_K_Y_INV);
+    MVD_CK(P.ly->strided_tma(a, dir, c->stream), "y pass (TMA)");
+  }
+  ++c->launches;
+  return MVD_OK;
+}
+
+mvd_status z_conv_tma(mvd_ctx* c, const float2* in, float2* out, const float2* spec, int xt0, int n_xt) {
+  const Plan& P = c->P;
+  ZconvTmaArgs a{};
+  if (!make_map3(&a.in_map, in, P.Mx, P.My, P.N[2], P.Mx, P.plane, P.Tzt, 1, P.zbox) ||
+      !make_map3(&a.spec_map, spec, P.Mx, P.My, P.Mz, P.Mx, P.plane, P.Tzt, 1, P.zbox)) {
+    snprintf(c->err, sizeof(c->err), "z pass: cuTensorMapEncodeTiled failed");
+    c->broken = true;
+    return MVD_ERR_CUDA;
+  }
+  a.out = out; a.tw = c->twz();
+  a.T = P.Tzt; a.nthreads = P.ntzt; a.boxr = P.zbox; a.nbox = P.znbox;
+  a.xt0 = xt0; a.n_xt = n_xt;
+  a.mx = P.Mx; a.my = P.My; a.plane = P.plane; a.nz = P.N[2];
+  if (c->zt_blocks == 0) c->zt_blocks = P.lz->zconv_tma_blocks_per_sm(a.nthreads, P.lz->zconv_tma_smem(a.T, a.boxr, a.nbox));
+  if (c->zt_blocks <= 0) { snprintf(c->err, sizeof(c->err), "z pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
+  a.grid = (int)std::min<long long>((long long)n_xt * P.My, (long long)c->num_sms * c->zt_blocks);
+  {
+    ProfScope ps(c, MVD_K_Z_CONV);
+    MVD_CK(P.lz->zconv_tma(a, c->stream), "z convolution pass (TMA)");
+  }
+  ++c->launches;
+  return MVD_OK;
+}
+
 // ---- pass launchers -------------------------------------------------------------------------
 mvd_status y_pass(mvd_ctx* c, float2* buf, int dir, int nz_planes, bool full) {
   const Plan& P = c->P;
+  if (P.ytma && !full) return y_pass_tma(c, buf, dir, nz_planes, 0, (P.Mx + P.Tyt - 1) / P.Tyt);
   StridedArgs a{};
   a.in = buf; a.out = buf; a.tw = c->twy();
   a.T = full ? P.Tys : P.Ty;
@@ -361,6 +483,7 @@ mvd_status z_plain_fwd(mvd_ctx* c, float2* buf) {
 
 mvd_status z_conv(mvd_ctx* c, const float2* in, float2* out, const float2* spec) {
   const Plan& P = c->P;
+  if (P.ztma) return z_conv_tma(c, in, out, spec, 0, (P.Mx + P.Tzt - 1) / P.Tzt);
   ZconvArgs a{};
   a.in = in; a.out = out; a.spec = spec; a.tw = c->twz();
   a.T = P.Tz; a.nthreads = P.ntz; a.plane = P.plane; a.nz = P.N[2];

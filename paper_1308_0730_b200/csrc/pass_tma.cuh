@@ -251,6 +251,206 @@ __global__ void __launch_bounds__(256) xrow_tma_kernel(const XArgs p) {
   }
 }
 
+// =========================================================================================
+// strided pencil FFT (form F), TMA-staged.  Tile = T contiguous complex elements x the whole
+// pencil, laid out [n][T] in shared memory by the tensor copy (rows >= n_in arrive as zeros:
+// the zero padding is never stored in HBM).  Both register transforms run in place on the tile:
+//   stage 1: item (n2, x) owns rows n1*B + n2 -> A-point FFT, twiddle -> rows k1*B + n2
+//   stage 2: item (k1, x) owns rows k1*B + n2 -> B-point FFT -> global rows k1 + A*k2 (< n_out)
+// =========================================================================================
+template <int A, int B, int DIR>
+__global__ void __launch_bounds__(PassCfg<A, B>::MAX_THREADS)
+strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
+  constexpr int M = A * B;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int T = p.T;
+  const int NR = p.boxr * p.nbox;
+  float2* buf = reinterpret_cast<float2*>(smem_raw);            // [2][NR][T]
+  float2* tws = buf + (size_t)2 * NR * T;                        // [M]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tws + M);
+  const int tid = threadIdx.x;
+  const int ntiles = p.n_xt * p.n_outer;
+
+  if (tid == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    mbar_fence_init();
+  }
+  for (int j = tid; j < M; j += blockDim.x) tws[j] = __ldg(p.tw + j);
+  __syncthreads();
+
+  auto issue = [&](int tile, int s) {
+    const int outer = tile / p.n_xt;
+    const int x0 = (p.xt0 + (tile - outer * p.n_xt)) * T;
+    mbar_expect_tx(&bars[s], (uint32_t)(NR * T * sizeof(float2)));
+    for (int b = 0; b < p.nbox; ++b)
+      tma_load_3d(buf + ((size_t)s * NR + b * p.boxr) * T, &p.in_map, x0, b * p.boxr, outer, &bars[s]);
+  };
+
+  if (tid == 0 && (int)blockIdx.x < ntiles) issue((int)blockIdx.x, 0);
+
+  int it = 0;
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+    const int s = it & 1;
+    float2* sm = buf + (size_t)s * NR * T;
+    if (tid == 0 && tile + (int)gridDim.x < ntiles) issue(tile + (int)gridDim.x, s ^ 1);
+    const int outer = tile / p.n_xt;
+    const int x0 = (p.xt0 + (tile - outer * p.n_xt)) * T;
+    const int xvalid = min(T, p.line_len - x0);
+    mbar_wait(&bars[s], (it >> 1) & 1);
+
+    for (int i = tid; i < T * B; i += blockDim.x) {
+      const int n2 = i / T;
+      float2 v[A];
+      static_for<0, A>([&](auto n1_) {
+        constexpr int n1 = decltype(n1_)::value;
+        v[n1] = sm[n1 * B * T + i];
+      });
+      FftReg<A, DIR>::run(v);
+      static_for<0, A>([&](auto k1_) {
+        constexpr int k1 = decltype(k1_)::value;
+        if constexpr (k1 > 0) {
+          const float2 w = tws[n2 * k1];
+          v[k1] = DIR < 0 ? cmul(v[k1], w) : cmul_conj(v[k1], w);
+        }
+        sm[k1 * B * T + i] = v[k1];
+      });
+    }
+    __syncthreads();
+    float2* out = p.out + (long long)outer * p.out_outer_stride + x0;
+    for (int j = tid; j < T * A; j += blockDim.x) {
+      const int k1 = j / T;
+      const int x = j - k1 * T;
+      float2 u[B];
+      static_for<0, B>([&](auto n2_) {
+        constexpr int n2 = decltype(n2_)::value;
+        u[n2] = sm[(k1 * B + n2) * T + x];
+      });
+      FftReg<B, DIR>::run(u);
+      if (x < xvalid) {
+        float2* o = out + (long long)k1 * p.out_pstride + x;
+        static_for<0, B>([&](auto k2_) {
+          constexpr int k2 = decltype(k2_)::value;
+          if (k1 + A * k2 < p.n_out) o[(long long)(A * k2) * p.out_pstride] = u[k2];
+        });
+      }
+    }
+    __syncthreads();   // the tile is free: the next iteration refills the other stage's partner
+  }
+}
+
+// =========================================================================================
+// fused z pass, TMA-staged: crop(IFFT_z( FFT_z(zero-padded pencil) * spectrum )).
+// Tile = T contiguous x of one row y, all z: the input tile [z][T] (planes >= nz arrive as zeros)
+// and the spectrum tile [k][T] are both staged by tensor copies; the four register transforms
+// run in place on the input tile.
+// =========================================================================================
+template <int A, int B>
+__global__ void __launch_bounds__(PassCfg<A, B>::MAX_THREADS)
+zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
+  constexpr int M = A * B;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int T = p.T;
+  const int NR = p.boxr * p.nbox;
+  float2* buf = reinterpret_cast<float2*>(smem_raw);            // [2][NR][T] input tiles
+  float2* sbuf = buf + (size_t)2 * NR * T;                       // [2][NR][T] spectrum tiles
+  float2* tws = sbuf + (size_t)2 * NR * T;                       // [M]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tws + M);
+  const int tid = threadIdx.x;
+  const int ntiles = p.n_xt * p.my;
+
+  if (tid == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    mbar_fence_init();
+  }
+  for (int j = tid; j < M; j += blockDim.x) tws[j] = __ldg(p.tw + j);
+  __syncthreads();
+
+  auto issue = [&](int tile, int s) {
+    const int y = tile / p.n_xt;
+    const int x0 = (p.xt0 + (tile - y * p.n_xt)) * T;
+    mbar_expect_tx(&bars[s], (uint32_t)(2 * NR * T * sizeof(float2)));
+    for (int b = 0; b < p.nbox; ++b) {
+      tma_load_3d(buf + ((size_t)s * NR + b * p.boxr) * T, &p.in_map, x0, y, b * p.boxr, &bars[s]);
+      tma_load_3d(sbuf + ((size_t)s * NR + b * p.boxr) * T, &p.spec_map, x0, y, b * p.boxr, &bars[s]);
+    }
+  };
+
+  if (tid == 0 && (int)blockIdx.x < ntiles) issue((int)blockIdx.x, 0);
+
+  int it = 0;
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+    const int s = it & 1;
+    float2* sm = buf + (size_t)s * NR * T;
+    const float2* sp = sbuf + (size_t)s * NR * T;
+    if (tid == 0 && tile + (int)gridDim.x < ntiles) issue(tile + (int)gridDim.x, s ^ 1);
+    const int y = tile / p.n_xt;
+    const int x0 = (p.xt0 + (tile - y * p.n_xt)) * T;
+    const int xvalid = min(T, p.mx - x0);
+    mbar_wait(&bars[s], (it >> 1) & 1);
+
+    // F1: item (n2, x), forward A-point transforms over n1
+    for (int i = tid; i < T * B; i += blockDim.x) {
+      const int n2 = i / T;
+      float2 v[A];
+      static_for<0, A>([&](auto n1_) {
+        constexpr int n1 = decltype(n1_)::value;
+        v[n1] = sm[n1 * B * T + i];
+      });
+      FftReg<A, -1>::run(v);
+      static_for<0, A>([&](auto k1_) {
+        constexpr int k1 = decltype(k1_)::value;
+        if constexpr (k1 > 0) v[k1] = cmul(v[k1], tws[n2 * k1]);
+        sm[k1 * B * T + i] = v[k1];
+      });
+    }
+    __syncthreads();
+    // F2 . spectrum . G1: item (k1, x)
+    for (int j = tid; j < T * A; j += blockDim.x) {
+      const int k1 = j / T;
+      const int x = j - k1 * T;
+      float2 u[B];
+      static_for<0, B>([&](auto n2_) {
+        constexpr int m = decltype(n2_)::value;
+        u[m] = sm[(k1 * B + m) * T + x];
+      });
+      FftReg<B, -1>::run(u);
+      static_for<0, B>([&](auto k2_) {
+        constexpr int k2 = decltype(k2_)::value;
+        u[k2] = cmul(u[k2], sp[(k1 + A * k2) * T + x]);
+      });
+      FftReg<B, 1>::run(u);
+      static_for<0, B>([&](auto n2_) {
+        constexpr int m = decltype(n2_)::value;
+        if constexpr (m > 0) u[m] = cmul_conj(u[m], tws[m * k1]);
+        sm[(k1 * B + m) * T + x] = u[m];
+      });
+    }
+    __syncthreads();
+    // G2: item (n2, x), inverse A-point transforms over k1, store planes n1*B + n2 < nz
+    float2* out = p.out + (long long)y * p.mx + x0;
+    for (int i = tid; i < T * B; i += blockDim.x) {
+      const int n2 = i / T;
+      const int x = i - n2 * T;
+      float2 v[A];
+      static_for<0, A>([&](auto k1_) {
+        constexpr int kk = decltype(k1_)::value;
+        v[kk] = sm[kk * B * T + i];
+      });
+      FftReg<A, 1>::run(v);
+      if (x < xvalid) {
+        float2* o = out + (long long)n2 * p.plane + x;
+        static_for<0, A>([&](auto n1_) {
+          constexpr int n1 = decltype(n1_)::value;
+          if (n1 * B + n2 < p.nz) o[(long long)(n1 * B) * p.plane] = v[n1];
+        });
+      }
+    }
+    __syncthreads();
+  }
+}
+
 // host-side launchers of the TMA-staged passes
 template <int A, int B>
 struct LaunchTma {
@@ -271,6 +471,9 @@ struct LaunchTma {
   if (e != cudaSuccess) { fprintf(stderr, "carveout attr failed %d x %d: %s\n", A, B, #k); return e; }
     MVD_SET((xrow_tma_kernel<A, B, X_QUOT>));
     MVD_SET((xrow_tma_kernel<A, B, X_UPDATE>));
+    MVD_SET((strided_tma_kernel<A, B, -1>));
+    MVD_SET((strided_tma_kernel<A, B, 1>));
+    MVD_SET((zconv_tma_kernel<A, B>));
 #undef MVD_SET
     return cudaSuccess;
   }
@@ -281,6 +484,37 @@ struct LaunchTma {
         ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_QUOT>, nthreads, smem)
         : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_UPDATE>, nthreads, smem);
     return e == cudaSuccess ? n : 0;
+  }
+
+  static size_t strided_smem(int T, int boxr, int nbox) {
+    return (size_t)2 * boxr * nbox * T * sizeof(float2) + (size_t)Cfg::M * sizeof(float2) + 16;
+  }
+  static size_t zconv_smem(int T, int boxr, int nbox) {
+    return (size_t)4 * boxr * nbox * T * sizeof(float2) + (size_t)Cfg::M * sizeof(float2) + 16;
+  }
+  static int strided_blocks_per_sm(int dir, int nthreads, size_t smem) {
+    int n = 0;
+    cudaError_t e = dir < 0
+        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, strided_tma_kernel<A, B, -1>, nthreads, smem)
+        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, strided_tma_kernel<A, B, 1>, nthreads, smem);
+    return e == cudaSuccess ? n : 0;
+  }
+  static int zconv_blocks_per_sm(int nthreads, size_t smem) {
+    int n = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, zconv_tma_kernel<A, B>, nthreads, smem);
+    return e == cudaSuccess ? n : 0;
+  }
+  static cudaError_t strided(const StridedTmaArgs& a, int dir, cudaStream_t s) {
+    if (a.grid <= 0) return cudaSuccess;
+    const size_t smem = strided_smem(a.T, a.boxr, a.nbox);
+    if (dir < 0) strided_tma_kernel<A, B, -1><<<a.grid, a.nthreads, smem, s>>>(a);
+    else strided_tma_kernel<A, B, 1><<<a.grid, a.nthreads, smem, s>>>(a);
+    return cudaGetLastError();
+  }
+  static cudaError_t zconv(const ZconvTmaArgs& a, cudaStream_t s) {
+    if (a.grid <= 0) return cudaSuccess;
+    zconv_tma_kernel<A, B><<<a.grid, a.nthreads, zconv_smem(a.T, a.boxr, a.nbox), s>>>(a);
+    return cudaGetLastError();
   }
 
   static cudaError_t xrow(const XArgs& a, int mode, cudaStream_t s) {
