@@ -8,6 +8,8 @@
 
 namespace mvd {
 
+constexpr int kTmaTileHost = 8;   // == kTmaTile of pass_tma.cuh
+
 // ---- TMA-staged strided pass (pass_tma.cuh): persistent CTAs, tiles of T contiguous complex
 //      elements x the whole pencil, loaded by tensor copies with zero fill beyond n_in ----------
 struct StridedTmaArgs {

@@ -15,14 +15,21 @@
 #include <type_traits>
 
 #ifdef MVD_HOST_TEST
+#include <cmath>
 struct float2 { float x, y; };
 static inline float2 make_float2(float a, float b) { return float2{a, b}; }
 #define MVD_DEV inline
 #define MVD_CE constexpr
+#define MVD_FMA(a, b, c) std::fmaf((a), (b), (c))
+#define MVD_MUL(a, b) ((a) * (b))
 #else
 #include <cuda_runtime.h>
 #define MVD_DEV __device__ __forceinline__
 #define MVD_CE __host__ __device__ constexpr
+// explicit rounding: the complex products contract the same way in every kernel, so the same
+// transform gives bit-identical results wherever it is inlined (resume == uninterrupted run)
+#define MVD_FMA(a, b, c) __fmaf_rn((a), (b), (c))
+#define MVD_MUL(a, b) __fmul_rn((a), (b))
 #endif
 
 namespace mvd {
@@ -81,10 +88,10 @@ MVD_CE cdouble ce_root(long long k, long long n) {   // exp(+2*pi*i*k/n)
 MVD_DEV float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 MVD_DEV float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 MVD_DEV float2 cmul(float2 a, float2 b) {
-  return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+  return make_float2(MVD_FMA(a.x, b.x, -MVD_MUL(a.y, b.y)), MVD_FMA(a.x, b.y, MVD_MUL(a.y, b.x)));
 }
 MVD_DEV float2 cmul_conj(float2 a, float2 b) {   // a * conj(b)
-  return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+  return make_float2(MVD_FMA(a.x, b.x, MVD_MUL(a.y, b.y)), MVD_FMA(a.y, b.x, -MVD_MUL(a.x, b.y)));
 }
 
 // multiply by exp(DIR * 2*pi*i * K / N), K and N compile-time (DIR = -1 forward, +1 inverse)
@@ -103,7 +110,7 @@ MVD_DEV float2 cmul_root(float2 a) {
     constexpr cdouble w = ce_root(k, N);
     constexpr float c = float(w.re);
     constexpr float s = float(DIR > 0 ? w.im : -w.im);
-    return make_float2(a.x * c - a.y * s, a.x * s + a.y * c);
+    return make_float2(MVD_FMA(a.x, c, -MVD_MUL(a.y, s)), MVD_FMA(a.x, s, MVD_MUL(a.y, c)));
   }
 }
 

@@ -195,7 +195,7 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
       const int boxr = ((l->M + nbox - 1) / nbox + 3) / 4 * 4;
       int best = 0;
       double best_score = -1.0;
-      const int cand[] = {8, 12, 16, 20, 24, 4};
+      const int cand[] = {kTmaTileHost};   // the kernels are compiled for one tile width
       for (int T : cand) {
         const size_t smem = zconv ? l->zconv_tma_smem(T, boxr, nbox) : l->strided_tma_smem(T, boxr, nbox);
         if (smem > smem_cap && T > 4) continue;
@@ -204,7 +204,8 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
         if (eff * seg > best_score + 1e-9) { best_score = eff * seg; best = T; }
       }
       if (best == 0) best = 4;
-      if (force > 0 && force % 4 == 0) best = force;
+      (void)force;
+      best = kTmaTileHost;
       const int items = best * ab;
       const int rounds = (items + l->max_threads - 1) / l->max_threads;
       *T_out = best;
@@ -223,11 +224,11 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
     // TMA-staged x pass (quotient / OSEM update): rows per tile sized for >= 3 resident CTAs per SM
     const int ab = std::max(P.lx->A, P.lx->B);
     P.xtma = env_int("MVD_XTMA", 1);
-    int R = std::max(1, 256 / ab);
+    int R = std::max(1, 160 / ab);   // kXrowTmaThreads of pass_tma.cuh
     const int force = env_int("MVD_RXT", 0);
-    const size_t cap = (size_t)env_int("MVD_XT_SMEM_KB", 72) * 1024;
+    const size_t cap = (size_t)env_int("MVD_XT_SMEM_KB", 45) * 1024;
     while (R > 1 && P.lx->xrow_tma_smem(R, P.r[0], P.N[0]) > cap) --R;
-    if (force > 0 && force * ab <= 256 && P.lx->xrow_tma_smem(force, P.r[0], P.N[0]) <= 220 * 1024) R = force;
+    if (force > 0 && force * ab <= 160 && P.lx->xrow_tma_smem(force, P.r[0], P.N[0]) <= 220 * 1024) R = force;
     if (P.lx->xrow_tma_smem(R, P.r[0], P.N[0]) > 220 * 1024) P.xtma = 0;
     P.Rxt = R;
     P.ntxt = round_up32(R * ab);

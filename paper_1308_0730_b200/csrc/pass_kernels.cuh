@@ -231,12 +231,9 @@ xrow_kernel(const XArgs p) {
         u[k2] = src[A * k2];
       });
       FftReg<B, 1>::run(u);
-      float2 pw[B];
-      const float2 w = ld_tw(p.tw, k1);
-      powers<B>(make_float2(w.x, -w.y), pw);          // conj(W)^{n2 k1}
       static_for<0, B>([&](auto n2_) {
         constexpr int m = decltype(n2_)::value;
-        if constexpr (m > 0) u[m] = cmul(u[m], pw[m]);
+        if constexpr (m > 0) u[m] = cmul_conj(u[m], ld_tw(p.tw, m * k1));   // conj(W)^{n2 k1}
         sm[rowA * RS + m * AP + k1] = u[m];
       });
     }
@@ -390,11 +387,9 @@ xrow_kernel(const XArgs p) {
   // ---- F1: forward A-point transforms over n1 ----------------------------------------------------
   if (actB) {
     FftReg<A, -1>::run(c);
-    float2 pw[A];
-    powers<A>(ld_tw(p.tw, n2), pw);                  // W^{n2 k1}
     static_for<0, A>([&](auto k1_) {
       constexpr int kk = decltype(k1_)::value;
-      if constexpr (kk > 0) c[kk] = cmul(c[kk], pw[kk]);
+      if constexpr (kk > 0) c[kk] = cmul(c[kk], ld_tw(p.tw, n2 * kk));   // W^{n2 k1}
       sm[rowB * RS + kk * BP + n2] = c[kk];
     });
   }

@@ -31,8 +31,14 @@ __host__ __device__ constexpr int xrow_rstride(int nx, int B) {
   return s;
 }
 
+// tile width (contiguous complex elements) of the TMA-staged y and z passes: compile-time, so every
+// shared-memory offset of the in-place transforms is an immediate
+constexpr int kTmaTile = 8;
+// thread cap of the TMA-staged x pass: 4+ resident CTAs per SM at <= 102 registers per thread
+constexpr int kXrowTmaThreads = 160;
+
 template <int A, int B, int MODE>
-__global__ void __launch_bounds__(256) xrow_tma_kernel(const XArgs p) {
+__global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArgs p) {
   using Cfg = PassCfg<A, B>;
   constexpr int M = Cfg::M, AP = Cfg::AP, BP = Cfg::BP, RS = Cfg::ROW_F2;
   constexpr int CS = xrow_cstride(M, A);
@@ -40,89 +46,96 @@ __global__ void __launch_bounds__(256) xrow_tma_kernel(const XArgs p) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int R = p.rows_per_cta;
   const int RSTR = p.real_stride;
-  // layout: [2 stages][R][CS] float2 | [2 stages][R][RSTR] float | exch [R][RS] float2 | halos | barriers
+  // layout: [R][CS] float2 complex rows | [R][RSTR] float real rows | exch [R][RS] float2 |
+  //         tw2 [M] float2 | halos | barriers.  One stage: each staging buffer is refilled for the
+  //         next tile as soon as its last reader of this tile has passed a barrier.
   float2* wst = reinterpret_cast<float2*>(smem_raw);
-  float* rst = reinterpret_cast<float*>(wst + (size_t)2 * R * CS);
-  float2* sm = reinterpret_cast<float2*>(rst + (size_t)2 * R * RSTR);
-  float* halo_re = reinterpret_cast<float*>(sm + (size_t)R * RS);
+  float* rst = reinterpret_cast<float*>(wst + (size_t)R * CS);
+  float2* sm = reinterpret_cast<float2*>(rst + (size_t)R * RSTR);
+  float2* tw2 = sm + (size_t)R * RS;                              // tw2[n2*A + k1] = W_M^(n2 k1)
+  float* halo_re = reinterpret_cast<float*>(tw2 + M);
   float* halo_im = halo_re + R * p.rx;
   uint64_t* bars = reinterpret_cast<uint64_t*>(
       (reinterpret_cast<uintptr_t>(halo_im + R * p.rx) + 7) & ~uintptr_t(7));
   const int tid = threadIdx.x;
   const float* real_src = MODE == X_QUOT ? p.phi : p.psi;
   const int ntiles = (int)((p.nrows + R - 1) / R);
+  const int nrows_i = (int)p.nrows;
 
   if (tid == 0) {
-    mbar_init(&bars[0], 1);
-    mbar_init(&bars[1], 1);
+    mbar_init(&bars[0], 1);   // complex rows landed
+    mbar_init(&bars[1], 1);   // real rows landed
     mbar_fence_init();
   }
+  for (int j = tid; j < M; j += blockDim.x) tw2[j] = __ldg(p.tw + (j / A) * (j % A));
   __syncthreads();
 
-  // warp 0 issues the copies of a tile: lane l stages complex and real rows l, l+32, ...
-  const int nrows_i = (int)p.nrows;
-  auto issue = [&](int tile, int s) {
+  // warp 0 issues the copies of a tile: lane l stages rows l, l+32, ...
+  auto issue_w = [&](int tile) {
     const int row0 = tile * R;
     const int rv = min(R, nrows_i - row0);
-    if (tid == 0)
-      mbar_expect_tx(&bars[s], (uint32_t)rv * (uint32_t)(M * sizeof(float2) + (p.bulk_real ? p.nx * sizeof(float) : 0)));
+    if (tid == 0) mbar_expect_tx(&bars[0], (uint32_t)rv * (uint32_t)(M * sizeof(float2)));
     __syncwarp();
     for (int r = tid; r < rv; r += 32) {
       const unsigned g = (unsigned)(row0 + r);
       const unsigned zq = g / (unsigned)p.ny_rows, yr = g - zq * (unsigned)p.ny_rows;
-      const long long off = (long long)zq * p.plane_pitch + (long long)yr * M;
-      bulk_g2s(wst + ((size_t)s * R + r) * CS, p.in + off, M * sizeof(float2), &bars[s]);
-      if (p.bulk_real)
-        bulk_g2s(rst + ((size_t)s * R + r) * RSTR, real_src + (long long)g * p.nx, p.nx * sizeof(float), &bars[s]);
+      bulk_g2s(wst + (size_t)r * CS, p.in + (long long)zq * p.plane_pitch + (long long)yr * M, M * sizeof(float2), &bars[0]);
     }
+  };
+  auto issue_r = [&](int tile) {
+    const int row0 = tile * R;
+    const int rv = min(R, nrows_i - row0);
+    if (tid == 0) mbar_expect_tx(&bars[1], (uint32_t)rv * (uint32_t)(p.nx * sizeof(float)));
+    __syncwarp();
+    for (int r = tid; r < rv; r += 32)
+      bulk_g2s(rst + (size_t)r * RSTR, real_src + (long long)(row0 + r) * p.nx, p.nx * sizeof(float), &bars[1]);
   };
 
   const int rowA = tid / A, k1 = tid - rowA * A;
   const int rowB = tid / B, n2 = tid - rowB * B;
   double dflux = 0.0, dl1 = 0.0;
 
-  if (tid < 32 && (int)blockIdx.x < ntiles) issue((int)blockIdx.x, 0);
+  if (tid < 32 && (int)blockIdx.x < ntiles) {
+    issue_w((int)blockIdx.x);
+    if (p.bulk_real) issue_r((int)blockIdx.x);
+  }
 
   int it = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
-    const int s = it & 1;
     const int row0 = tile * R;
     const int growA = row0 + rowA, growB = row0 + rowB;
     const bool actA = tid < R * A && growA < nrows_i;
     const bool actB = tid < R * B && growB < nrows_i;
-    // stage s^1 was last read before the barriers of the previous tile: refill it now
-    if (tid < 32 && tile + (int)gridDim.x < ntiles) issue(tile + (int)gridDim.x, s ^ 1);
+    const bool more = tile + (int)gridDim.x < ntiles;
     if (!p.bulk_real) {   // rows not 16-byte aligned: plain loads of this tile's real rows
       const int rv = min(R, nrows_i - row0);
       for (int i = tid; i < rv * p.nx; i += blockDim.x) {
         const int r = i / p.nx, x = i - r * p.nx;
-        rst[((size_t)s * R + r) * RSTR + x] = real_src[(long long)(row0 + r) * p.nx + x];
+        rst[(size_t)r * RSTR + x] = real_src[(long long)(row0 + r) * p.nx + x];
       }
-      __syncthreads();
     }
-    mbar_wait(&bars[s], (it >> 1) & 1);
+    mbar_wait(&bars[0], it & 1);
 
     float2 c[A];
     float flux = 0.f, l1 = 0.f;
     // ---- G1: inverse B-point transforms over k2 ------------------------------------------------
     if (actA) {
       float2 u[B];
-      const float2* src = wst + ((size_t)s * R + rowA) * CS + k1;
+      const float2* src = wst + (size_t)rowA * CS + k1;
       static_for<0, B>([&](auto k2_) {
         constexpr int k2 = decltype(k2_)::value;
         u[k2] = src[A * k2];
       });
       FftReg<B, 1>::run(u);
-      float2 pw[B];
-      const float2 w = ld_tw(p.tw, k1);
-      powers<B>(make_float2(w.x, -w.y), pw);
       static_for<0, B>([&](auto n2_) {
         constexpr int m = decltype(n2_)::value;
-        if constexpr (m > 0) u[m] = cmul(u[m], pw[m]);
+        if constexpr (m > 0) u[m] = cmul_conj(u[m], tw2[m * A + k1]);
         sm[rowA * RS + m * AP + k1] = u[m];
       });
     }
     __syncthreads();
+    // every G1 read of the complex rows is done: stage the next tile's
+    if (tid < 32 && more) issue_w(tile + (int)gridDim.x);
     // ---- G2: inverse A-point transforms over k1 -> c[n1], n = n1*B + n2 ------------------------
     if (actB) {
       static_for<0, A>([&](auto k1_) {
@@ -141,10 +154,11 @@ __global__ void __launch_bounds__(256) xrow_tma_kernel(const XArgs p) {
       });
     }
     __syncthreads();
+    if (p.bulk_real) mbar_wait(&bars[1], it & 1);
     // ---- pointwise stage on the real row -------------------------------------------------------
     if (actB) {
       const long long rbase = (long long)growB * p.nx;
-      const float* rrow = rst + ((size_t)s * R + rowB) * RSTR;
+      const float* rrow = rst + (size_t)rowB * RSTR;
       float* prow = p.psi + rbase;
       const int lo_int = p.rx, hi_int = min(p.hx - p.rx, p.nx - p.hx);   // interior: no overlap, both halves live
       static_for<0, A>([&](auto n1_) {
@@ -193,15 +207,15 @@ __global__ void __launch_bounds__(256) xrow_tma_kernel(const XArgs p) {
       });
       // ---- F1: forward A-point transforms over n1 ----------------------------------------------
       FftReg<A, -1>::run(c);
-      float2 pw[A];
-      powers<A>(ld_tw(p.tw, n2), pw);
       static_for<0, A>([&](auto k1_) {
         constexpr int kk = decltype(k1_)::value;
-        if constexpr (kk > 0) c[kk] = cmul(c[kk], pw[kk]);
+        if constexpr (kk > 0) c[kk] = cmul(c[kk], tw2[n2 * A + kk]);
         sm[rowB * RS + kk * BP + n2] = c[kk];
       });
     }
     __syncthreads();
+    // every read of the real rows is done: stage the next tile's
+    if (tid < 32 && more && p.bulk_real) issue_r(tile + (int)gridDim.x);
     // ---- F2: forward B-point transforms over n2, store k = k1 + A*k2 ---------------------------
     if (actA) {
       float2 u[B];
@@ -263,7 +277,7 @@ __global__ void __launch_bounds__(PassCfg<A, B>::MAX_THREADS)
 strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
   constexpr int M = A * B;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  const int T = p.T;
+  constexpr int T = kTmaTile;
   const int NR = p.boxr * p.nbox;
   float2* buf = reinterpret_cast<float2*>(smem_raw);            // [2][NR][T]
   float2* tws = buf + (size_t)2 * NR * T;                        // [M]
@@ -276,7 +290,7 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
     mbar_init(&bars[1], 1);
     mbar_fence_init();
   }
-  for (int j = tid; j < M; j += blockDim.x) tws[j] = __ldg(p.tw + j);
+  for (int j = tid; j < M; j += blockDim.x) tws[j] = __ldg(p.tw + (j / A) * (j % A));   // tws[n2*A + k1] = W^(n2 k1)
   __syncthreads();
 
   auto issue = [&](int tile, int s) {
@@ -310,7 +324,7 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
       static_for<0, A>([&](auto k1_) {
         constexpr int k1 = decltype(k1_)::value;
         if constexpr (k1 > 0) {
-          const float2 w = tws[n2 * k1];
+          const float2 w = tws[n2 * A + k1];
           v[k1] = DIR < 0 ? cmul(v[k1], w) : cmul_conj(v[k1], w);
         }
         sm[k1 * B * T + i] = v[k1];
@@ -350,7 +364,7 @@ __global__ void __launch_bounds__(PassCfg<A, B>::MAX_THREADS)
 zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
   constexpr int M = A * B;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  const int T = p.T;
+  constexpr int T = kTmaTile;
   const int NR = p.boxr * p.nbox;
   float2* buf = reinterpret_cast<float2*>(smem_raw);            // [2][NR][T] input tiles
   float2* sbuf = buf + (size_t)2 * NR * T;                       // [2][NR][T] spectrum tiles
@@ -364,7 +378,7 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
     mbar_init(&bars[1], 1);
     mbar_fence_init();
   }
-  for (int j = tid; j < M; j += blockDim.x) tws[j] = __ldg(p.tw + j);
+  for (int j = tid; j < M; j += blockDim.x) tws[j] = __ldg(p.tw + (j / A) * (j % A));   // tws[n2*A + k1] = W^(n2 k1)
   __syncthreads();
 
   auto issue = [&](int tile, int s) {
@@ -401,7 +415,7 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
       FftReg<A, -1>::run(v);
       static_for<0, A>([&](auto k1_) {
         constexpr int k1 = decltype(k1_)::value;
-        if constexpr (k1 > 0) v[k1] = cmul(v[k1], tws[n2 * k1]);
+        if constexpr (k1 > 0) v[k1] = cmul(v[k1], tws[n2 * A + k1]);
         sm[k1 * B * T + i] = v[k1];
       });
     }
@@ -423,7 +437,7 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
       FftReg<B, 1>::run(u);
       static_for<0, B>([&](auto n2_) {
         constexpr int m = decltype(n2_)::value;
-        if constexpr (m > 0) u[m] = cmul_conj(u[m], tws[m * k1]);
+        if constexpr (m > 0) u[m] = cmul_conj(u[m], tws[m * A + k1]);
         sm[(k1 * B + m) * T + x] = u[m];
       });
     }
@@ -457,9 +471,9 @@ struct LaunchTma {
   using Cfg = PassCfg<A, B>;
 
   static size_t xrow_smem(int rows, int rx, int nx) {
-    return (size_t)2 * rows * xrow_cstride(Cfg::M, A) * sizeof(float2) +
-           (size_t)2 * rows * xrow_rstride(nx, B) * sizeof(float) + (size_t)rows * Cfg::ROW_F2 * sizeof(float2) +
-           (size_t)2 * rows * rx * sizeof(float) + 32;
+    return (size_t)rows * xrow_cstride(Cfg::M, A) * sizeof(float2) +
+           (size_t)rows * xrow_rstride(nx, B) * sizeof(float) + (size_t)rows * Cfg::ROW_F2 * sizeof(float2) +
+           (size_t)Cfg::M * sizeof(float2) + (size_t)2 * rows * rx * sizeof(float) + 32;
   }
 
   static cudaError_t init() {
