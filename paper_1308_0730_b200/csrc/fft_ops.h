@@ -37,6 +37,7 @@ struct ZconvTmaArgs {
   int mx, my;              // row length and rows per plane
   long long plane;         // elements between z planes of `out`
   int nz;                  // planes written
+  int nst_in;              // shared-memory stages of the input tile: 1 or 2
 };
 
 // ---- strided pencil FFT (y pass, plain z pass): pencils along a strided axis, tiles of T
@@ -120,7 +121,7 @@ struct LengthOps {
   size_t (*strided_tma_smem)(int T, int boxr, int nbox);
   int (*strided_tma_blocks_per_sm)(int dir, int nthreads, size_t smem);
   cudaError_t (*zconv_tma)(const ZconvTmaArgs&, cudaStream_t);
-  size_t (*zconv_tma_smem)(int T, int boxr, int nbox);
+  size_t (*zconv_tma_smem)(int T, int boxr, int nbox, int nst_in);
   int (*zconv_tma_blocks_per_sm)(int nthreads, size_t smem);
 };
 

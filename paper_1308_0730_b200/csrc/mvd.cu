@@ -88,7 +88,7 @@ struct Plan {
   int xtma = 0, Rxt = 0, ntxt = 0, xt_rstride = 0;
   // TMA-staged y and z passes: tile width, threads, pencil boxes (boxr rows x nbox >= M)
   int ytma = 0, Tyt = 0, ntyt = 0, ybox = 0, ynbox = 0;
-  int ztma = 0, Tzt = 0, ntzt = 0, zbox = 0, znbox = 0;
+  int ztma = 0, Tzt = 0, ntzt = 0, zbox = 0, znbox = 0, znst = 2;
   // workspace offsets (bytes)
   size_t off_twx = 0, off_twy = 0, off_twz = 0, off_psi = 0, off_acc = 0, off_w = 0, off_w0 = 0,
          off_spec = 0, off_psf = 0, off_kern = 0, off_auto = 0, off_stage = 0, off_partials = 0,
@@ -197,7 +197,7 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
       double best_score = -1.0;
       const int cand[] = {kTmaTileHost};   // the kernels are compiled for one tile width
       for (int T : cand) {
-        const size_t smem = zconv ? l->zconv_tma_smem(T, boxr, nbox) : l->strided_tma_smem(T, boxr, nbox);
+        const size_t smem = zconv ? l->zconv_tma_smem(T, boxr, nbox, P.znst) : l->strided_tma_smem(T, boxr, nbox);
         if (smem > smem_cap && T > 4) continue;
         const double eff = double(L) / double(((L + T - 1) / T) * T);
         const double seg = T >= 8 ? 1.0 : 0.7;
@@ -206,15 +206,16 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
       if (best == 0) best = 4;
       (void)force;
       best = kTmaTileHost;
-      const int items = best * ab;
+      const int items = best * ab * (zconv ? 2 : 1);   // the z tile is 8 x by 2 rows
       const int rounds = (items + l->max_threads - 1) / l->max_threads;
       *T_out = best;
       *nt_out = std::min(l->max_threads, round_up32((items + rounds - 1) / rounds));
       *box_out = boxr;
       *nbox_out = nbox;
-      const size_t smem = zconv ? l->zconv_tma_smem(best, boxr, nbox) : l->strided_tma_smem(best, boxr, nbox);
+      const size_t smem = zconv ? l->zconv_tma_smem(best, boxr, nbox, P.znst) : l->strided_tma_smem(best, boxr, nbox);
       return smem <= 220 * 1024;
     };
+    P.znst = env_int("MVD_ZNST", 2) == 1 ? 1 : 2;
     P.ytma = env_int("MVD_YTMA", 1);
     P.ztma = env_int("MVD_ZTMA", 1);
     if (!plan_tma(P.ly, P.Mx, env_int("MVD_TYT", 0), (size_t)env_int("MVD_YT_SMEM_KB", 72) * 1024, false, &P.Tyt, &P.ntyt, &P.ybox, &P.ynbox)) P.ytma = 0;
@@ -421,8 +422,8 @@ mvd_status y_pass_tma(mvd_ctx* c, float2* buf, int dir, int nz_planes, int xt0, 
 mvd_status z_conv_tma(mvd_ctx* c, const float2* in, float2* out, const float2* spec, int xt0, int n_xt) {
   const Plan& P = c->P;
   ZconvTmaArgs a{};
-  if (!make_map3(&a.in_map, in, P.Mx, P.My, P.N[2], P.Mx, P.plane, P.Tzt, 1, P.zbox) ||
-      !make_map3(&a.spec_map, spec, P.Mx, P.My, P.Mz, P.Mx, P.plane, P.Tzt, 1, P.zbox)) {
+  if (!make_map3(&a.in_map, in, P.Mx, P.My, P.N[2], P.Mx, P.plane, P.Tzt, 2, P.zbox) ||
+      !make_map3(&a.spec_map, spec, P.Mx, P.My, P.Mz, P.Mx, P.plane, P.Tzt, 2, P.zbox)) {
     snprintf(c->err, sizeof(c->err), "z pass: cuTensorMapEncodeTiled failed");
     c->broken = true;
     return MVD_ERR_CUDA;
@@ -430,10 +431,10 @@ mvd_status z_conv_tma(mvd_ctx* c, const float2* in, float2* out, const float2* s
   a.out = out; a.tw = c->twz();
   a.T = P.Tzt; a.nthreads = P.ntzt; a.boxr = P.zbox; a.nbox = P.znbox;
   a.xt0 = xt0; a.n_xt = n_xt;
-  a.mx = P.Mx; a.my = P.My; a.plane = P.plane; a.nz = P.N[2];
-  if (c->zt_blocks == 0) c->zt_blocks = P.lz->zconv_tma_blocks_per_sm(a.nthreads, P.lz->zconv_tma_smem(a.T, a.boxr, a.nbox));
+  a.mx = P.Mx; a.my = P.My; a.plane = P.plane; a.nz = P.N[2]; a.nst_in = P.znst;
+  if (c->zt_blocks == 0) c->zt_blocks = P.lz->zconv_tma_blocks_per_sm(a.nthreads, P.lz->zconv_tma_smem(a.T, a.boxr, a.nbox, a.nst_in));
   if (c->zt_blocks <= 0) { snprintf(c->err, sizeof(c->err), "z pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
-  a.grid = (int)std::min<long long>((long long)n_xt * P.My, (long long)c->num_sms * c->zt_blocks);
+  a.grid = (int)std::min<long long>((long long)n_xt * ((P.My + 1) / 2), (long long)c->num_sms * c->zt_blocks);
   {
     ProfScope ps(c, MVD_K_Z_CONV);
     MVD_CK(P.lz->zconv_tma(a, c->stream), "z convolution pass (TMA)");

@@ -364,45 +364,62 @@ __global__ void __launch_bounds__(PassCfg<A, B>::MAX_THREADS)
 zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
   constexpr int M = A * B;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  constexpr int T = kTmaTile;
+  constexpr int TX = kTmaTile, T = 2 * kTmaTile;   // tile: 8 contiguous x of two consecutive rows y
   const int NR = p.boxr * p.nbox;
-  float2* buf = reinterpret_cast<float2*>(smem_raw);            // [2][NR][T] input tiles
-  float2* sbuf = buf + (size_t)2 * NR * T;                       // [2][NR][T] spectrum tiles
-  float2* tws = sbuf + (size_t)2 * NR * T;                       // [M]
-  uint64_t* bars = reinterpret_cast<uint64_t*>(tws + M);
+  const int nst = p.nst_in;                                       // input stages: 1 or 2
+  float2* buf = reinterpret_cast<float2*>(smem_raw);            // [nst][NR][T] input tiles
+  float2* sbuf = buf + (size_t)nst * NR * T;                     // [NR][T] spectrum tile (one stage)
+  float2* tws = sbuf + (size_t)NR * T;                           // [M]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tws + M);        // [0..1] input stages, [2] spectrum
   const int tid = threadIdx.x;
-  const int ntiles = p.n_xt * p.my;
+  const int ny2 = (p.my + 1) / 2;                                 // row pairs
+  const int ntiles = p.n_xt * ny2;
 
   if (tid == 0) {
     mbar_init(&bars[0], 1);
     mbar_init(&bars[1], 1);
+    mbar_init(&bars[2], 1);
     mbar_fence_init();
   }
   for (int j = tid; j < M; j += blockDim.x) tws[j] = __ldg(p.tw + (j / A) * (j % A));   // tws[n2*A + k1] = W^(n2 k1)
   __syncthreads();
 
-  auto issue = [&](int tile, int s) {
-    const int y = tile / p.n_xt;
-    const int x0 = (p.xt0 + (tile - y * p.n_xt)) * T;
-    mbar_expect_tx(&bars[s], (uint32_t)(2 * NR * T * sizeof(float2)));
-    for (int b = 0; b < p.nbox; ++b) {
+  auto issue_in = [&](int tile, int s) {
+    const int yp = tile / p.n_xt;
+    const int y = 2 * yp;
+    const int x0 = (p.xt0 + (tile - yp * p.n_xt)) * TX;
+    mbar_expect_tx(&bars[s], (uint32_t)(NR * T * sizeof(float2)));
+    for (int b = 0; b < p.nbox; ++b)
       tma_load_3d(buf + ((size_t)s * NR + b * p.boxr) * T, &p.in_map, x0, y, b * p.boxr, &bars[s]);
-      tma_load_3d(sbuf + ((size_t)s * NR + b * p.boxr) * T, &p.spec_map, x0, y, b * p.boxr, &bars[s]);
-    }
+  };
+  auto issue_spec = [&](int tile) {
+    const int yp = tile / p.n_xt;
+    const int y = 2 * yp;
+    const int x0 = (p.xt0 + (tile - yp * p.n_xt)) * TX;
+    mbar_expect_tx(&bars[2], (uint32_t)(NR * T * sizeof(float2)));
+    for (int b = 0; b < p.nbox; ++b)
+      tma_load_3d(sbuf + (size_t)(b * p.boxr) * T, &p.spec_map, x0, y, b * p.boxr, &bars[2]);
   };
 
-  if (tid == 0 && (int)blockIdx.x < ntiles) issue((int)blockIdx.x, 0);
+  if (tid == 0 && (int)blockIdx.x < ntiles) {
+    issue_in((int)blockIdx.x, 0);
+    issue_spec((int)blockIdx.x);
+  }
 
   int it = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
-    const int s = it & 1;
+    const int s = nst == 2 ? (it & 1) : 0;
     float2* sm = buf + (size_t)s * NR * T;
-    const float2* sp = sbuf + (size_t)s * NR * T;
-    if (tid == 0 && tile + (int)gridDim.x < ntiles) issue(tile + (int)gridDim.x, s ^ 1);
-    const int y = tile / p.n_xt;
-    const int x0 = (p.xt0 + (tile - y * p.n_xt)) * T;
-    const int xvalid = min(T, p.mx - x0);
-    mbar_wait(&bars[s], (it >> 1) & 1);
+    const float2* sp = sbuf;
+    const bool more = tile + (int)gridDim.x < ntiles;
+    // two input stages: the other stage was last read before the final barrier of the previous tile
+    if (tid == 0 && more && nst == 2) issue_in(tile + (int)gridDim.x, s ^ 1);
+    const int yp = tile / p.n_xt;
+    const int y = 2 * yp;
+    const int x0 = (p.xt0 + (tile - yp * p.n_xt)) * TX;
+    const int xvalid = min(TX, p.mx - x0);
+    const int yvalid = min(2, p.my - y);
+    mbar_wait(&bars[s], nst == 2 ? ((it >> 1) & 1) : (it & 1));
 
     // F1: item (n2, x), forward A-point transforms over n1
     for (int i = tid; i < T * B; i += blockDim.x) {
@@ -420,6 +437,7 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
       });
     }
     __syncthreads();
+    mbar_wait(&bars[2], it & 1);
     // F2 . spectrum . G1: item (k1, x)
     for (int j = tid; j < T * A; j += blockDim.x) {
       const int k1 = j / T;
@@ -442,19 +460,22 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
       });
     }
     __syncthreads();
+    // every read of the spectrum tile is done: stage the next tile's
+    if (tid == 0 && more) issue_spec(tile + (int)gridDim.x);
     // G2: item (n2, x), inverse A-point transforms over k1, store planes n1*B + n2 < nz
     float2* out = p.out + (long long)y * p.mx + x0;
     for (int i = tid; i < T * B; i += blockDim.x) {
       const int n2 = i / T;
-      const int x = i - n2 * T;
+      const int col = i - n2 * T;
+      const int yy = col / TX, x = col - yy * TX;
       float2 v[A];
       static_for<0, A>([&](auto k1_) {
         constexpr int kk = decltype(k1_)::value;
         v[kk] = sm[kk * B * T + i];
       });
       FftReg<A, 1>::run(v);
-      if (x < xvalid) {
-        float2* o = out + (long long)n2 * p.plane + x;
+      if (x < xvalid && yy < yvalid) {
+        float2* o = out + (long long)n2 * p.plane + yy * p.mx + x;
         static_for<0, A>([&](auto n1_) {
           constexpr int n1 = decltype(n1_)::value;
           if (n1 * B + n2 < p.nz) o[(long long)(n1 * B) * p.plane] = v[n1];
@@ -462,6 +483,7 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
       }
     }
     __syncthreads();
+    if (tid == 0 && more && nst == 1) issue_in(tile + (int)gridDim.x, 0);   // one input stage: refill now
   }
 }
 
@@ -503,8 +525,8 @@ struct LaunchTma {
   static size_t strided_smem(int T, int boxr, int nbox) {
     return (size_t)2 * boxr * nbox * T * sizeof(float2) + (size_t)Cfg::M * sizeof(float2) + 16;
   }
-  static size_t zconv_smem(int T, int boxr, int nbox) {
-    return (size_t)4 * boxr * nbox * T * sizeof(float2) + (size_t)Cfg::M * sizeof(float2) + 16;
+  static size_t zconv_smem(int T, int boxr, int nbox, int nst_in) {   // T = 8 x 2 rows = 16 columns
+    return (size_t)(nst_in + 1) * boxr * nbox * 2 * T * sizeof(float2) + (size_t)Cfg::M * sizeof(float2) + 32;
   }
   static int strided_blocks_per_sm(int dir, int nthreads, size_t smem) {
     int n = 0;
@@ -527,7 +549,7 @@ struct LaunchTma {
   }
   static cudaError_t zconv(const ZconvTmaArgs& a, cudaStream_t s) {
     if (a.grid <= 0) return cudaSuccess;
-    zconv_tma_kernel<A, B><<<a.grid, a.nthreads, zconv_smem(a.T, a.boxr, a.nbox), s>>>(a);
+    zconv_tma_kernel<A, B><<<a.grid, a.nthreads, zconv_smem(a.T, a.boxr, a.nbox, a.nst_in), s>>>(a);
     return cudaGetLastError();
   }
 
