@@ -8,7 +8,10 @@
 
 namespace mvd {
 
-constexpr int kTmaTileHost = 8;   // == kTmaTile of pass_tma.cuh
+#ifndef MVD_TMA_TILE
+#define MVD_TMA_TILE 8
+#endif
+constexpr int kTmaTileHost = MVD_TMA_TILE;   // == kTmaTile of pass_tma.cuh
 
 // ---- TMA-staged strided pass (pass_tma.cuh): persistent CTAs, tiles of T contiguous complex
 //      elements x the whole pencil, loaded by tensor copies with zero fill beyond n_in ----------
@@ -102,6 +105,9 @@ struct XArgs {
   int real_stride;         // floats between real rows in shared memory
   int bulk_real;           // real rows are 16-byte aligned: staged by bulk copies (else plain loads)
   int grid;                // persistent CTAs
+  int exch_stride;         // float2 per row of the exchange buffer (allocation)
+  int exch_stride_g;       // row stride of the inverse-side exchange layout [n2*AP + k1]
+  int exch_stride_f;       // row stride of the forward-side exchange layout [k1*BP + n2]
 };
 
 struct LengthOps {

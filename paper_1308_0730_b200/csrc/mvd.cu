@@ -85,7 +85,7 @@ struct Plan {
   int Ty = 0, nty = 0, Tz = 0, ntz = 0, Tzs = 0, ntzs = 0, Tys = 0, ntys = 0, Rx = 0, ntx = 0;
   int nctax = 0;
   // TMA-staged x pass
-  int xtma = 0, Rxt = 0, ntxt = 0, xt_rstride = 0;
+  int xtma = 0, Rxt = 0, ntxt = 0, xt_rstride = 0, xt_exch = 0, xt_exch_g = 0, xt_exch_f = 0;
   // TMA-staged y and z passes: tile width, threads, pencil boxes (boxr rows x nbox >= M)
   int ytma = 0, Tyt = 0, ntyt = 0, ybox = 0, ynbox = 0;
   int ztma = 0, Tzt = 0, ntzt = 0, zbox = 0, znbox = 0, znst = 2;
@@ -96,6 +96,46 @@ struct Plan {
   size_t psf_stride = 0, auto_stride = 0;   // elements (doubles) per view
   int sum_blocks = 0;
 };
+
+// Shared-memory wavefronts of the x pass's exchange buffer for one row stride: 64-bit accesses are
+// served per half-warp, one wavefront per distinct bank pair multiplicity.  g_layout: rows written by
+// (row, k1) lanes at [m*AP + k1] and read by (row, n2) lanes at [n2*AP + kk]; else the forward layout
+// [k1*BP + m] / [kk*BP + n2].
+static long long exch_wavefronts(int A, int B, int R, int nthreads, int RS, bool g_layout) {
+  const int AP = A | 1, BP = B | 1;
+  long long total = 0;
+  for (int hw = 0; hw < nthreads / 16; ++hw) {
+    for (int pass = 0; pass < 2; ++pass) {
+      const int role = pass == 0 ? A : B;          // lanes per row
+      const int reps = pass == 0 ? B : A;          // unrolled accesses per thread
+      for (int m = 0; m < reps; ++m) {
+        int cnt[16] = {0};
+        int worst = 0;
+        for (int l = 0; l < 16; ++l) {
+          const int t = hw * 16 + l;
+          if (t >= R * role) continue;
+          const int row = t / role, q = t % role;
+          int addr;
+          if (g_layout) addr = pass == 0 ? row * RS + m * AP + q : row * RS + q * AP + m;
+          else addr = pass == 0 ? row * RS + q * BP + m : row * RS + m * BP + q;
+          worst = std::max(worst, ++cnt[addr & 15]);
+        }
+        total += worst;
+      }
+    }
+  }
+  return total;
+}
+
+static int best_exch_stride(int A, int B, int R, int nthreads, int min_stride, bool g_layout) {
+  int best = min_stride;
+  long long best_cost = -1;
+  for (int rs = min_stride; rs < min_stride + 16; ++rs) {
+    const long long cst = exch_wavefronts(A, B, R, nthreads, rs, g_layout);
+    if (best_cost < 0 || cst < best_cost) { best_cost = cst; best = rs; }
+  }
+  return best;
+}
 
 static int env_int(const char* name, int dflt) {
   const char* s = getenv(name);
@@ -237,6 +277,11 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
     const int want = (P.lx->B % 32) / 4 * 4;
     while ((s % 32) != want) s += 4;
     P.xt_rstride = s;
+    const int A = P.lx->A, B = P.lx->B;
+    const int row_min = std::max(A * (B | 1), B * (A | 1));
+    P.xt_exch = row_min + 16;
+    P.xt_exch_g = best_exch_stride(A, B, R, P.ntxt, B * (A | 1), true);
+    P.xt_exch_f = best_exch_stride(A, B, R, P.ntxt, A * (B | 1), false);
   }
 
   // workspace layout
@@ -409,6 +454,7 @@ mvd_status y_pass_tma(mvd_ctx* c, float2* buf, int dir, int nz_planes, int xt0, 
   a.n_out = dir < 0 ? P.My : P.N[1];
   int& bl = c->yt_blocks[dir < 0 ? 0 : 1];
   if (bl == 0) bl = P.ly->strided_tma_blocks_per_sm(dir, a.nthreads, P.ly->strided_tma_smem(a.T, a.boxr, a.nbox));
+  if (env_int("MVD_YBLK", 0) > 0) bl = std::min(bl, env_int("MVD_YBLK", 0));
   if (bl <= 0) { snprintf(c->err, sizeof(c->err), "y pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
   a.grid = (int)std::min<long long>((long long)n_xt * nz_planes, (long long)c->num_sms * bl);
   {
@@ -433,6 +479,7 @@ mvd_status z_conv_tma(mvd_ctx* c, const float2* in, float2* out, const float2* s
   a.xt0 = xt0; a.n_xt = n_xt;
   a.mx = P.Mx; a.my = P.My; a.plane = P.plane; a.nz = P.N[2]; a.nst_in = P.znst;
   if (c->zt_blocks == 0) c->zt_blocks = P.lz->zconv_tma_blocks_per_sm(a.nthreads, P.lz->zconv_tma_smem(a.T, a.boxr, a.nbox, a.nst_in));
+  if (env_int("MVD_ZBLK", 0) > 0) c->zt_blocks = std::min(c->zt_blocks, env_int("MVD_ZBLK", 0));
   if (c->zt_blocks <= 0) { snprintf(c->err, sizeof(c->err), "z pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
   a.grid = (int)std::min<long long>((long long)n_xt * ((P.My + 1) / 2), (long long)c->num_sms * c->zt_blocks);
   {
@@ -522,10 +569,12 @@ mvd_status x_pass(mvd_ctx* c, const XArgs& a_in, int mode) {
     a.rows_per_cta = P.Rxt;
     a.nthreads = P.ntxt;
     a.real_stride = P.xt_rstride;
+    a.exch_stride = P.xt_exch; a.exch_stride_g = P.xt_exch_g; a.exch_stride_f = P.xt_exch_f;
     const float* real_src = mode == X_QUOT ? a.phi : a.psi;
     a.bulk_real = (P.N[0] % 4 == 0) && ((reinterpret_cast<size_t>(real_src) & 15) == 0);
     if (c->xt_blocks[mode] == 0) {
       c->xt_blocks[mode] = P.lx->xrow_tma_blocks_per_sm(mode, a.nthreads, P.lx->xrow_tma_smem(a.rows_per_cta, P.r[0], P.N[0]));
+      if (env_int("MVD_XBLK", 0) > 0) c->xt_blocks[mode] = std::min(c->xt_blocks[mode], env_int("MVD_XBLK", 0));
       if (c->xt_blocks[mode] <= 0) { snprintf(c->err, sizeof(c->err), "x pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
     }
     const long long ntiles = (a.nrows + a.rows_per_cta - 1) / a.rows_per_cta;

@@ -33,27 +33,28 @@ __host__ __device__ constexpr int xrow_rstride(int nx, int B) {
 
 // tile width (contiguous complex elements) of the TMA-staged y and z passes: compile-time, so every
 // shared-memory offset of the in-place transforms is an immediate
-constexpr int kTmaTile = 8;
+constexpr int kTmaTile = kTmaTileHost;
 // thread cap of the TMA-staged x pass: 4+ resident CTAs per SM at <= 102 registers per thread
 constexpr int kXrowTmaThreads = 160;
 
 template <int A, int B, int MODE>
 __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArgs p) {
   using Cfg = PassCfg<A, B>;
-  constexpr int M = Cfg::M, AP = Cfg::AP, BP = Cfg::BP, RS = Cfg::ROW_F2;
+  constexpr int M = Cfg::M, AP = Cfg::AP, BP = Cfg::BP;
   constexpr int CS = xrow_cstride(M, A);
   static_assert(MODE == X_QUOT || MODE == X_UPDATE, "TMA-staged x pass: quotient and OSEM update only");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int R = p.rows_per_cta;
   const int RSTR = p.real_stride;
+  const int RS = p.exch_stride, RSG = p.exch_stride_g, RSF = p.exch_stride_f;
   // layout: [R][CS] float2 complex rows | [R][RSTR] float real rows | exch [R][RS] float2 |
   //         tw2 [M] float2 | halos | barriers.  One stage: each staging buffer is refilled for the
   //         next tile as soon as its last reader of this tile has passed a barrier.
   float2* wst = reinterpret_cast<float2*>(smem_raw);
   float* rst = reinterpret_cast<float*>(wst + (size_t)R * CS);
   float2* sm = reinterpret_cast<float2*>(rst + (size_t)R * RSTR);
-  float2* tw2 = sm + (size_t)R * RS;                              // tw2[n2*A + k1] = W_M^(n2 k1)
-  float* halo_re = reinterpret_cast<float*>(tw2 + M);
+  float2* tw2 = sm + (size_t)R * RS;                              // tw2[n2*AP + k1] = W_M^(n2 k1)
+  float* halo_re = reinterpret_cast<float*>(tw2 + B * AP);
   float* halo_im = halo_re + R * p.rx;
   uint64_t* bars = reinterpret_cast<uint64_t*>(
       (reinterpret_cast<uintptr_t>(halo_im + R * p.rx) + 7) & ~uintptr_t(7));
@@ -67,7 +68,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
     mbar_init(&bars[1], 1);   // real rows landed
     mbar_fence_init();
   }
-  for (int j = tid; j < M; j += blockDim.x) tw2[j] = __ldg(p.tw + (j / A) * (j % A));
+  for (int j = tid; j < M; j += blockDim.x) tw2[(j / A) * AP + (j % A)] = __ldg(p.tw + (j / A) * (j % A));
   __syncthreads();
 
   // warp 0 issues the copies of a tile: lane l stages rows l, l+32, ...
@@ -129,8 +130,8 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
       FftReg<B, 1>::run(u);
       static_for<0, B>([&](auto n2_) {
         constexpr int m = decltype(n2_)::value;
-        if constexpr (m > 0) u[m] = cmul_conj(u[m], tw2[m * A + k1]);
-        sm[rowA * RS + m * AP + k1] = u[m];
+        if constexpr (m > 0) u[m] = cmul_conj(u[m], tw2[m * AP + k1]);
+        sm[rowA * RSG + m * AP + k1] = u[m];
       });
     }
     __syncthreads();
@@ -140,7 +141,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
     if (actB) {
       static_for<0, A>([&](auto k1_) {
         constexpr int kk = decltype(k1_)::value;
-        c[kk] = sm[rowB * RS + n2 * AP + kk];
+        c[kk] = sm[rowB * RSG + n2 * AP + kk];
       });
       FftReg<A, 1>::run(c);
       static_for<0, A>([&](auto n1_) {
@@ -209,8 +210,8 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
       FftReg<A, -1>::run(c);
       static_for<0, A>([&](auto k1_) {
         constexpr int kk = decltype(k1_)::value;
-        if constexpr (kk > 0) c[kk] = cmul(c[kk], tw2[n2 * A + kk]);
-        sm[rowB * RS + kk * BP + n2] = c[kk];
+        if constexpr (kk > 0) c[kk] = cmul(c[kk], tw2[n2 * AP + kk]);
+        sm[rowB * RSF + kk * BP + n2] = c[kk];
       });
     }
     __syncthreads();
@@ -221,7 +222,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
       float2 u[B];
       static_for<0, B>([&](auto n2_) {
         constexpr int m = decltype(n2_)::value;
-        u[m] = sm[rowA * RS + k1 * BP + m];
+        u[m] = sm[rowA * RSF + k1 * BP + m];
       });
       FftReg<B, -1>::run(u);
       const unsigned zq = (unsigned)growA / (unsigned)p.ny_rows, yr = (unsigned)growA - zq * (unsigned)p.ny_rows;
@@ -280,8 +281,9 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
   constexpr int T = kTmaTile;
   const int NR = p.boxr * p.nbox;
   float2* buf = reinterpret_cast<float2*>(smem_raw);            // [2][NR][T]
-  float2* tws = buf + (size_t)2 * NR * T;                        // [M]
-  uint64_t* bars = reinterpret_cast<uint64_t*>(tws + M);
+  constexpr int AP = PassCfg<A, B>::AP;
+  float2* tws = buf + (size_t)2 * NR * T;                        // [B][AP]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tws + B * AP);
   const int tid = threadIdx.x;
   const int ntiles = p.n_xt * p.n_outer;
 
@@ -290,7 +292,7 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
     mbar_init(&bars[1], 1);
     mbar_fence_init();
   }
-  for (int j = tid; j < M; j += blockDim.x) tws[j] = __ldg(p.tw + (j / A) * (j % A));   // tws[n2*A + k1] = W^(n2 k1)
+  for (int j = tid; j < M; j += blockDim.x) tws[(j / A) * AP + (j % A)] = __ldg(p.tw + (j / A) * (j % A));   // tws[n2*AP + k1] = W^(n2 k1)
   __syncthreads();
 
   auto issue = [&](int tile, int s) {
@@ -324,7 +326,7 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
       static_for<0, A>([&](auto k1_) {
         constexpr int k1 = decltype(k1_)::value;
         if constexpr (k1 > 0) {
-          const float2 w = tws[n2 * A + k1];
+          const float2 w = tws[n2 * AP + k1];
           v[k1] = DIR < 0 ? cmul(v[k1], w) : cmul_conj(v[k1], w);
         }
         sm[k1 * B * T + i] = v[k1];
@@ -369,8 +371,9 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
   const int nst = p.nst_in;                                       // input stages: 1 or 2
   float2* buf = reinterpret_cast<float2*>(smem_raw);            // [nst][NR][T] input tiles
   float2* sbuf = buf + (size_t)nst * NR * T;                     // [NR][T] spectrum tile (one stage)
-  float2* tws = sbuf + (size_t)NR * T;                           // [M]
-  uint64_t* bars = reinterpret_cast<uint64_t*>(tws + M);        // [0..1] input stages, [2] spectrum
+  constexpr int AP = PassCfg<A, B>::AP;
+  float2* tws = sbuf + (size_t)NR * T;                           // [B][AP]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tws + B * AP);   // [0..1] input stages, [2] spectrum
   const int tid = threadIdx.x;
   const int ny2 = (p.my + 1) / 2;                                 // row pairs
   const int ntiles = p.n_xt * ny2;
@@ -381,7 +384,7 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
     mbar_init(&bars[2], 1);
     mbar_fence_init();
   }
-  for (int j = tid; j < M; j += blockDim.x) tws[j] = __ldg(p.tw + (j / A) * (j % A));   // tws[n2*A + k1] = W^(n2 k1)
+  for (int j = tid; j < M; j += blockDim.x) tws[(j / A) * AP + (j % A)] = __ldg(p.tw + (j / A) * (j % A));   // tws[n2*AP + k1] = W^(n2 k1)
   __syncthreads();
 
   auto issue_in = [&](int tile, int s) {
@@ -432,7 +435,7 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
       FftReg<A, -1>::run(v);
       static_for<0, A>([&](auto k1_) {
         constexpr int k1 = decltype(k1_)::value;
-        if constexpr (k1 > 0) v[k1] = cmul(v[k1], tws[n2 * A + k1]);
+        if constexpr (k1 > 0) v[k1] = cmul(v[k1], tws[n2 * AP + k1]);
         sm[k1 * B * T + i] = v[k1];
       });
     }
@@ -455,7 +458,7 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
       FftReg<B, 1>::run(u);
       static_for<0, B>([&](auto n2_) {
         constexpr int m = decltype(n2_)::value;
-        if constexpr (m > 0) u[m] = cmul_conj(u[m], tws[m * A + k1]);
+        if constexpr (m > 0) u[m] = cmul_conj(u[m], tws[m * AP + k1]);
         sm[(k1 * B + m) * T + x] = u[m];
       });
     }
@@ -492,10 +495,11 @@ template <int A, int B>
 struct LaunchTma {
   using Cfg = PassCfg<A, B>;
 
+  // exchange rows are at most ROW_F2 + 16 float2 (the planner searches the conflict-free stride there)
   static size_t xrow_smem(int rows, int rx, int nx) {
     return (size_t)rows * xrow_cstride(Cfg::M, A) * sizeof(float2) +
-           (size_t)rows * xrow_rstride(nx, B) * sizeof(float) + (size_t)rows * Cfg::ROW_F2 * sizeof(float2) +
-           (size_t)Cfg::M * sizeof(float2) + (size_t)2 * rows * rx * sizeof(float) + 32;
+           (size_t)rows * xrow_rstride(nx, B) * sizeof(float) + (size_t)rows * (Cfg::ROW_F2 + 16) * sizeof(float2) +
+           (size_t)B * Cfg::AP * sizeof(float2) + (size_t)2 * rows * rx * sizeof(float) + 32;
   }
 
   static cudaError_t init() {
@@ -523,10 +527,10 @@ struct LaunchTma {
   }
 
   static size_t strided_smem(int T, int boxr, int nbox) {
-    return (size_t)2 * boxr * nbox * T * sizeof(float2) + (size_t)Cfg::M * sizeof(float2) + 16;
+    return (size_t)2 * boxr * nbox * T * sizeof(float2) + (size_t)B * Cfg::AP * sizeof(float2) + 16;
   }
   static size_t zconv_smem(int T, int boxr, int nbox, int nst_in) {   // T = 8 x 2 rows = 16 columns
-    return (size_t)(nst_in + 1) * boxr * nbox * 2 * T * sizeof(float2) + (size_t)Cfg::M * sizeof(float2) + 32;
+    return (size_t)(nst_in + 1) * boxr * nbox * 2 * T * sizeof(float2) + (size_t)B * Cfg::AP * sizeof(float2) + 32;
   }
   static int strided_blocks_per_sm(int dir, int nthreads, size_t smem) {
     int n = 0;
