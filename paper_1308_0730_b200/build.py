@@ -22,6 +22,8 @@ LIB = os.path.join(HERE, "libmvd.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-Xfatbin=-compress-all"]
+if os.environ.get("MVD_SKIP_MATH"):   # experiment: memory traffic only (results are wrong)
+    FLAGS += ["-DMVD_SKIP_MATH"]
 if os.environ.get("MVD_TMA_TILE"):   # experiment: tile width of the TMA-staged y/z passes
     FLAGS += ["-DMVD_TMA_TILE=" + os.environ["MVD_TMA_TILE"]]
 

@@ -26,6 +26,7 @@ struct StridedTmaArgs {
   int n_outer;
   long long out_outer_stride, out_pstride;
   int n_out;               // pencil outputs >= n_out are not stored
+  int reverse;             // walk the tiles last to first (reads what the previous pass wrote last: L2 hits)
 };
 
 // ---- TMA-staged fused z pass: input tile and spectrum tile by tensor copies --------------------
@@ -58,6 +59,7 @@ struct StridedArgs {
   long long in_pstride, out_pstride;   // element stride along the pencil
   int n_in;                // pencil inputs >= n_in are zero (never read)
   int n_out;               // pencil outputs >= n_out are not stored
+  int reverse;             // walk the tiles last to first (reads what the previous pass wrote last: L2 hits)
 };
 
 // ---- fused z pass: forward FFT along z, multiply by a kernel spectrum, inverse FFT ----------
@@ -105,6 +107,7 @@ struct XArgs {
   int real_stride;         // floats between real rows in shared memory
   int bulk_real;           // real rows are 16-byte aligned: staged by bulk copies (else plain loads)
   int grid;                // persistent CTAs
+  int reverse;             // walk the tiles last to first
   int exch_stride;         // float2 per row of the exchange buffer (allocation)
   int exch_stride_g;       // row stride of the inverse-side exchange layout [n2*AP + k1]
   int exch_stride_f;       // row stride of the forward-side exchange layout [k1*BP + n2]

@@ -341,6 +341,8 @@ struct mvd_ctx {
   char err[512] = {0};
   int num_sms = 148;
   int xt_blocks[4] = {0, 0, 0, 0};   // resident CTAs per SM of the TMA-staged x pass, per mode
+  int flip = 0;                      // tile direction of the next x / y launch (alternates: L2 reuse)
+  int use_flip = 1;
   int yt_blocks[2] = {0, 0};         // ... of the TMA-staged y pass (forward, inverse)
   int zt_blocks = 0;                 // ... of the TMA-staged z pass
   // per-kernel-class event timing (mvd_profile)
@@ -452,6 +454,7 @@ mvd_status y_pass_tma(mvd_ctx* c, float2* buf, int dir, int nz_planes, int xt0, 
   a.line_len = P.Mx; a.n_outer = nz_planes;
   a.out_outer_stride = P.plane; a.out_pstride = P.Mx;
   a.n_out = dir < 0 ? P.My : P.N[1];
+  a.reverse = c->use_flip ? (c->flip ^= 1) : 0;
   int& bl = c->yt_blocks[dir < 0 ? 0 : 1];
   if (bl == 0) bl = P.ly->strided_tma_blocks_per_sm(dir, a.nthreads, P.ly->strided_tma_smem(a.T, a.boxr, a.nbox));
   if (env_int("MVD_YBLK", 0) > 0) bl = std::min(bl, env_int("MVD_YBLK", 0));
@@ -569,6 +572,7 @@ mvd_status x_pass(mvd_ctx* c, const XArgs& a_in, int mode) {
     a.rows_per_cta = P.Rxt;
     a.nthreads = P.ntxt;
     a.real_stride = P.xt_rstride;
+    a.reverse = c->use_flip ? (c->flip ^= 1) : 0;
     a.exch_stride = P.xt_exch; a.exch_stride_g = P.xt_exch_g; a.exch_stride_f = P.xt_exch_f;
     const float* real_src = mode == X_QUOT ? a.phi : a.psi;
     a.bulk_real = (P.N[0] % 4 == 0) && ((reinterpret_cast<size_t>(real_src) & 15) == 0);
@@ -852,6 +856,7 @@ mvd_status mvd_create(mvd_ctx** out, int n_views, const float* const* views, con
   c->stream = reinterpret_cast<cudaStream_t>(opt->stream);
   c->ws = reinterpret_cast<char*>(opt->workspace);
   c->use_graph = opt->use_graph;
+  c->use_flip = env_int("MVD_FLIP", 1);
   if (c->use_graph && !c->stream) {   // the legacy default stream cannot be captured
     fprintf(stderr, "mvd_create: use_graph needs a non-default stream\n");
     delete c;

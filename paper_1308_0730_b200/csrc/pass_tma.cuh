@@ -72,7 +72,8 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
   __syncthreads();
 
   // warp 0 issues the copies of a tile: lane l stages rows l, l+32, ...
-  auto issue_w = [&](int tile) {
+  auto issue_w = [&](int t) {
+    const int tile = p.reverse ? ntiles - 1 - t : t;
     const int row0 = tile * R;
     const int rv = min(R, nrows_i - row0);
     if (tid == 0) mbar_expect_tx(&bars[0], (uint32_t)rv * (uint32_t)(M * sizeof(float2)));
@@ -83,7 +84,8 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
       bulk_g2s(wst + (size_t)r * CS, p.in + (long long)zq * p.plane_pitch + (long long)yr * M, M * sizeof(float2), &bars[0]);
     }
   };
-  auto issue_r = [&](int tile) {
+  auto issue_r = [&](int t) {
+    const int tile = p.reverse ? ntiles - 1 - t : t;
     const int row0 = tile * R;
     const int rv = min(R, nrows_i - row0);
     if (tid == 0) mbar_expect_tx(&bars[1], (uint32_t)rv * (uint32_t)(p.nx * sizeof(float)));
@@ -103,7 +105,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
 
   int it = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
-    const int row0 = tile * R;
+    const int row0 = (p.reverse ? ntiles - 1 - tile : tile) * R;
     const int growA = row0 + rowA, growB = row0 + rowB;
     const bool actA = tid < R * A && growA < nrows_i;
     const bool actB = tid < R * B && growB < nrows_i;
@@ -295,7 +297,8 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
   for (int j = tid; j < M; j += blockDim.x) tws[(j / A) * AP + (j % A)] = __ldg(p.tw + (j / A) * (j % A));   // tws[n2*AP + k1] = W^(n2 k1)
   __syncthreads();
 
-  auto issue = [&](int tile, int s) {
+  auto issue = [&](int t, int s) {
+    const int tile = p.reverse ? ntiles - 1 - t : t;
     const int outer = tile / p.n_xt;
     const int x0 = (p.xt0 + (tile - outer * p.n_xt)) * T;
     mbar_expect_tx(&bars[s], (uint32_t)(NR * T * sizeof(float2)));
@@ -310,8 +313,9 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
     const int s = it & 1;
     float2* sm = buf + (size_t)s * NR * T;
     if (tid == 0 && tile + (int)gridDim.x < ntiles) issue(tile + (int)gridDim.x, s ^ 1);
-    const int outer = tile / p.n_xt;
-    const int x0 = (p.xt0 + (tile - outer * p.n_xt)) * T;
+    const int rtile = p.reverse ? ntiles - 1 - tile : tile;
+    const int outer = rtile / p.n_xt;
+    const int x0 = (p.xt0 + (rtile - outer * p.n_xt)) * T;
     const int xvalid = min(T, p.line_len - x0);
     mbar_wait(&bars[s], (it >> 1) & 1);
 
