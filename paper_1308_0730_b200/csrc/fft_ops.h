@@ -27,6 +27,7 @@ struct StridedTmaArgs {
   long long out_outer_stride, out_pstride;
   int n_out;               // pencil outputs >= n_out are not stored
   int reverse;             // walk the tiles last to first (reads what the previous pass wrote last: L2 hits)
+  int nst;                 // shared-memory stages of the tile: 1 or 2
 };
 
 // ---- TMA-staged fused z pass: input tile and spectrum tile by tensor copies --------------------
@@ -60,6 +61,7 @@ struct StridedArgs {
   int n_in;                // pencil inputs >= n_in are zero (never read)
   int n_out;               // pencil outputs >= n_out are not stored
   int reverse;             // walk the tiles last to first (reads what the previous pass wrote last: L2 hits)
+  int nst;                 // shared-memory stages of the tile: 1 or 2
 };
 
 // ---- fused z pass: forward FFT along z, multiply by a kernel spectrum, inverse FFT ----------
@@ -127,7 +129,7 @@ struct LengthOps {
   size_t (*xrow_tma_smem)(int rows, int rx, int nx);
   int (*xrow_tma_blocks_per_sm)(int mode, int nthreads, size_t smem);
   cudaError_t (*strided_tma)(const StridedTmaArgs&, int dir, cudaStream_t);
-  size_t (*strided_tma_smem)(int T, int boxr, int nbox);
+  size_t (*strided_tma_smem)(int T, int boxr, int nbox, int nst);
   int (*strided_tma_blocks_per_sm)(int dir, int nthreads, size_t smem);
   cudaError_t (*zconv_tma)(const ZconvTmaArgs&, cudaStream_t);
   size_t (*zconv_tma_smem)(int T, int boxr, int nbox, int nst_in);

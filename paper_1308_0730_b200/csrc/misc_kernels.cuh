@@ -109,24 +109,31 @@ __global__ void __launch_bounds__(128) autocorr_kernel(const double* __restrict_
 
 // kern[j] *= sum_u flipPv[u] G[off + j - u],  flipPv[u] = Pv[K-1-u], off = (Gd-1)/2, j in the box of
 // P_v: the central crop of the full convolution P_v* (*) G (R6).  G = P_w (*) P_w* (eq. 105) or P_w (eq. 107).
+// One warp per output tap: the lanes share the (uz, uy) rows of the sum, then a shuffle reduction.
 __global__ void __launch_bounds__(128) corr_crop_mul_kernel(const double* __restrict__ Pv, Dims3 K,
                                                             const double* __restrict__ G, Dims3 Gd,
                                                             double* __restrict__ kern) {
   const long long tot = (long long)K.x * K.y * K.z;
-  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long j = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;   // warp-uniform
   if (j >= tot) return;
+  const int lane = threadIdx.x & 31;
   const int jx = int(j % K.x), jy = int((j / K.x) % K.y), jz = int(j / ((long long)K.x * K.y));
   const int ox = (Gd.x - 1) / 2 + jx, oy = (Gd.y - 1) / 2 + jy, oz = (Gd.z - 1) / 2 + jz;
-  double acc = 0.0;
   // g index = o - u in [0, Gd)  ->  u in (o - Gd, o]
-  for (int uz = max(0, oz - Gd.z + 1); uz <= min(K.z - 1, oz); ++uz)
-    for (int uy = max(0, oy - Gd.y + 1); uy <= min(K.y - 1, oy); ++uy) {
-      const double* pv = Pv + ((long long)(K.z - 1 - uz) * K.y + (K.y - 1 - uy)) * K.x;
-      const double* g = G + ((long long)(oz - uz) * Gd.y + (oy - uy)) * Gd.x;
-      for (int ux = max(0, ox - Gd.x + 1); ux <= min(K.x - 1, ox); ++ux)
-        acc += pv[K.x - 1 - ux] * g[ox - ux];
-    }
-  kern[j] *= acc;
+  const int uz0 = max(0, oz - Gd.z + 1), uz1 = min(K.z - 1, oz);
+  const int uy0 = max(0, oy - Gd.y + 1), uy1 = min(K.y - 1, oy);
+  const int ux0 = max(0, ox - Gd.x + 1), ux1 = min(K.x - 1, ox);
+  const int nyr = uy1 - uy0 + 1;
+  const int nrows = (uz1 - uz0 + 1) * nyr;
+  double acc = 0.0;
+  for (int r = lane; r < nrows; r += 32) {
+    const int uz = uz0 + r / nyr, uy = uy0 + r % nyr;
+    const double* pv = Pv + ((long long)(K.z - 1 - uz) * K.y + (K.y - 1 - uy)) * K.x;
+    const double* g = G + ((long long)(oz - uz) * Gd.y + (oy - uy)) * Gd.x;
+    for (int ux = ux0; ux <= ux1; ++ux) acc += pv[K.x - 1 - ux] * g[ox - ux];
+  }
+  acc = warp_sum(acc);
+  if (lane == 0) kern[j] *= acc;
 }
 
 // kern[j] = (P[K-1-j])^power  (mirror, L312; power = V gives eq. 108, R9)

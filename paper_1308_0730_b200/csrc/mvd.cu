@@ -87,7 +87,7 @@ struct Plan {
   // TMA-staged x pass
   int xtma = 0, Rxt = 0, ntxt = 0, xt_rstride = 0, xt_exch = 0, xt_exch_g = 0, xt_exch_f = 0;
   // TMA-staged y and z passes: tile width, threads, pencil boxes (boxr rows x nbox >= M)
-  int ytma = 0, Tyt = 0, ntyt = 0, ybox = 0, ynbox = 0;
+  int ytma = 0, Tyt = 0, ntyt = 0, ybox = 0, ynbox = 0, ynst = 2;
   int ztma = 0, Tzt = 0, ntzt = 0, zbox = 0, znbox = 0, znst = 2;
   // workspace offsets (bytes)
   size_t off_twx = 0, off_twy = 0, off_twz = 0, off_psi = 0, off_acc = 0, off_w = 0, off_w0 = 0,
@@ -237,7 +237,7 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
       double best_score = -1.0;
       const int cand[] = {kTmaTileHost};   // the kernels are compiled for one tile width
       for (int T : cand) {
-        const size_t smem = zconv ? l->zconv_tma_smem(T, boxr, nbox, P.znst) : l->strided_tma_smem(T, boxr, nbox);
+        const size_t smem = zconv ? l->zconv_tma_smem(T, boxr, nbox, P.znst) : l->strided_tma_smem(T, boxr, nbox, P.ynst);
         if (smem > smem_cap && T > 4) continue;
         const double eff = double(L) / double(((L + T - 1) / T) * T);
         const double seg = T >= 8 ? 1.0 : 0.7;
@@ -252,10 +252,21 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
       *nt_out = std::min(l->max_threads, round_up32((items + rounds - 1) / rounds));
       *box_out = boxr;
       *nbox_out = nbox;
-      const size_t smem = zconv ? l->zconv_tma_smem(best, boxr, nbox, P.znst) : l->strided_tma_smem(best, boxr, nbox);
+      const size_t smem = zconv ? l->zconv_tma_smem(best, boxr, nbox, P.znst) : l->strided_tma_smem(best, boxr, nbox, P.ynst);
       return smem <= 220 * 1024;
     };
     P.znst = env_int("MVD_ZNST", 2) == 1 ? 1 : 2;
+    {
+      // two tile stages whenever they fit (one stage with more CTAs per SM measured slower on config 5)
+      const int nbox = (P.ly->M + 255) / 256;
+      const int boxr = ((P.ly->M + nbox - 1) / nbox + 3) / 4 * 4;
+      P.ynst = P.ly->strided_tma_smem(kTmaTileHost, boxr, nbox, 2) <= 200 * 1024 ? 2 : 1;
+      const int force = env_int("MVD_YNST", 0);
+      if (force == 1 || force == 2) P.ynst = force;
+      const int nbz = (P.lz->M + 255) / 256;
+      const int bxz = ((P.lz->M + nbz - 1) / nbz + 3) / 4 * 4;
+      if (env_int("MVD_ZNST", 0) == 0) P.znst = P.lz->zconv_tma_smem(kTmaTileHost, bxz, nbz, 2) <= 200 * 1024 ? 2 : 1;
+    }
     P.ytma = env_int("MVD_YTMA", 1);
     P.ztma = env_int("MVD_ZTMA", 1);
     if (!plan_tma(P.ly, P.Mx, env_int("MVD_TYT", 0), (size_t)env_int("MVD_YT_SMEM_KB", 72) * 1024, false, &P.Tyt, &P.ntyt, &P.ybox, &P.ynbox)) P.ytma = 0;
@@ -450,13 +461,13 @@ mvd_status y_pass_tma(mvd_ctx* c, float2* buf, int dir, int nz_planes, int xt0, 
   }
   a.out = buf; a.tw = c->twy();
   a.T = P.Tyt; a.nthreads = P.ntyt; a.boxr = P.ybox; a.nbox = P.ynbox;
-  a.xt0 = xt0; a.n_xt = n_xt;
+  a.xt0 = xt0; a.n_xt = n_xt; a.nst = P.ynst;
   a.line_len = P.Mx; a.n_outer = nz_planes;
   a.out_outer_stride = P.plane; a.out_pstride = P.Mx;
   a.n_out = dir < 0 ? P.My : P.N[1];
   a.reverse = c->use_flip ? (c->flip ^= 1) : 0;
   int& bl = c->yt_blocks[dir < 0 ? 0 : 1];
-  if (bl == 0) bl = P.ly->strided_tma_blocks_per_sm(dir, a.nthreads, P.ly->strided_tma_smem(a.T, a.boxr, a.nbox));
+  if (bl == 0) bl = P.ly->strided_tma_blocks_per_sm(dir, a.nthreads, P.ly->strided_tma_smem(a.T, a.boxr, a.nbox, a.nst));
   if (env_int("MVD_YBLK", 0) > 0) bl = std::min(bl, env_int("MVD_YBLK", 0));
   if (bl <= 0) { snprintf(c->err, sizeof(c->err), "y pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
   a.grid = (int)std::min<long long>((long long)n_xt * nz_planes, (long long)c->num_sms * bl);
@@ -734,7 +745,7 @@ mvd_status precompute(mvd_ctx* c, const float* const* psfs_host) {
   for (int v = 0; v < P.V; ++v) {
     const Dims3 K = P.K[v];
     const long long tot = (long long)K.x * K.y * K.z;
-    const unsigned g256 = (unsigned)((tot + 255) / 256), g128 = (unsigned)((tot + 127) / 128);
+    const unsigned g256 = (unsigned)((tot + 255) / 256), g128 = (unsigned)((tot + 3) / 4);   // corr: one warp per tap
     flip_pow_kernel<<<g256, 256, 0, c->stream>>>(c->psf(v), K, P.kmode == MVD_KERNEL_OPT2 ? P.V : 1, c->kern(v));
     MVD_CK(cudaGetLastError(), "flip_pow_kernel");
     ++c->launches;

@@ -282,9 +282,10 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int T = kTmaTile;
   const int NR = p.boxr * p.nbox;
-  float2* buf = reinterpret_cast<float2*>(smem_raw);            // [2][NR][T]
+  const int nst = p.nst;                                          // tile stages: 1 or 2
+  float2* buf = reinterpret_cast<float2*>(smem_raw);            // [nst][NR][T]
   constexpr int AP = PassCfg<A, B>::AP;
-  float2* tws = buf + (size_t)2 * NR * T;                        // [B][AP]
+  float2* tws = buf + (size_t)nst * NR * T;                        // [B][AP]
   uint64_t* bars = reinterpret_cast<uint64_t*>(tws + B * AP);
   const int tid = threadIdx.x;
   const int ntiles = p.n_xt * p.n_outer;
@@ -310,14 +311,15 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
 
   int it = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
-    const int s = it & 1;
+    const int s = nst == 2 ? (it & 1) : 0;
     float2* sm = buf + (size_t)s * NR * T;
-    if (tid == 0 && tile + (int)gridDim.x < ntiles) issue(tile + (int)gridDim.x, s ^ 1);
+    const bool more = tile + (int)gridDim.x < ntiles;
+    if (tid == 0 && more && nst == 2) issue(tile + (int)gridDim.x, s ^ 1);
     const int rtile = p.reverse ? ntiles - 1 - tile : tile;
     const int outer = rtile / p.n_xt;
     const int x0 = (p.xt0 + (rtile - outer * p.n_xt)) * T;
     const int xvalid = min(T, p.line_len - x0);
-    mbar_wait(&bars[s], (it >> 1) & 1);
+    mbar_wait(&bars[s], nst == 2 ? ((it >> 1) & 1) : (it & 1));
 
     for (int i = tid; i < T * B; i += blockDim.x) {
       const int n2 = i / T;
@@ -355,7 +357,8 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
         });
       }
     }
-    __syncthreads();   // the tile is free: the next iteration refills the other stage's partner
+    __syncthreads();   // every read of this tile is done
+    if (tid == 0 && more && nst == 1) issue(tile + (int)gridDim.x, 0);   // one stage: refill it now
   }
 }
 
@@ -530,8 +533,8 @@ struct LaunchTma {
     return e == cudaSuccess ? n : 0;
   }
 
-  static size_t strided_smem(int T, int boxr, int nbox) {
-    return (size_t)2 * boxr * nbox * T * sizeof(float2) + (size_t)B * Cfg::AP * sizeof(float2) + 16;
+  static size_t strided_smem(int T, int boxr, int nbox, int nst) {
+    return (size_t)nst * boxr * nbox * T * sizeof(float2) + (size_t)B * Cfg::AP * sizeof(float2) + 16;
   }
   static size_t zconv_smem(int T, int boxr, int nbox, int nst_in) {   // T = 8 x 2 rows = 16 columns
     return (size_t)(nst_in + 1) * boxr * nbox * 2 * T * sizeof(float2) + (size_t)B * Cfg::AP * sizeof(float2) + 32;
@@ -550,7 +553,7 @@ struct LaunchTma {
   }
   static cudaError_t strided(const StridedTmaArgs& a, int dir, cudaStream_t s) {
     if (a.grid <= 0) return cudaSuccess;
-    const size_t smem = strided_smem(a.T, a.boxr, a.nbox);
+    const size_t smem = strided_smem(a.T, a.boxr, a.nbox, a.nst);
     if (dir < 0) strided_tma_kernel<A, B, -1><<<a.grid, a.nthreads, smem, s>>>(a);
     else strided_tma_kernel<A, B, 1><<<a.grid, a.nthreads, smem, s>>>(a);
     return cudaGetLastError();
