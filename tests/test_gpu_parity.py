@@ -315,3 +315,62 @@ def test_blocked_single_block_equals_whole(mvd, tiny):
     got, _ = mvd.deconvolve_blocked(to_dev(tiny.views), tiny.psfs, (64, 64, 64), 2, variant="efficient")
     whole, _ = gpu_checkpoints(mvd, tiny, "efficient", "auto", (2,))
     assert np.array_equal(got.cpu().numpy(), whole[2])
+
+
+# ------------------------------------------------------------------------------------------
+# BASELINE config 4 at full size, in the launch configuration bench.py times (CUDA graph replay)
+# ------------------------------------------------------------------------------------------
+def test_config4_bench_configuration(mvd):
+    """512x512x256, 7 views, efficient-OSEM, one CUDA graph per iteration: every voxel against the
+    oracle after 1 and 2 iterations (14 view-updates; the oracle needs ~15 s per iteration)."""
+    p = mvd_synth.make_problem(4)
+    g, st = gpu_checkpoints(mvd, p, "osem", "auto", (1, 2), use_graph=True)
+    o, orc = oracle_checkpoints(p, "osem", "auto", (1, 2))
+    check(g[1], o[1], 1, "config 4")
+    l2, mx = errors(g[2], o[2])
+    assert l2 <= 2e-5 and mx <= TOL_MAX, (l2, mx)      # 2 iterations: well inside the 10-iteration bound
+    assert st["flux"] == pytest.approx(orc.flux, rel=1e-5)
+
+
+# ------------------------------------------------------------------------------------------
+# BASELINE config 5 size (1024x1024x512, PSF 25x25x51): the oracle cannot run the whole volume in
+# seconds, so (i) one 'same' convolution is checked at sampled voxels against the direct-sum
+# definition (O1) and (ii) the flux identity P3, which holds at any size, is checked after one update
+# ------------------------------------------------------------------------------------------
+def test_config5_size_sampled_voxels_and_flux(mvd):
+    import torch
+    dims, box = (1024, 1024, 512), (25, 25, 51)
+    nx, ny, nz = dims
+    rng = np.random.default_rng([13080730, 5, 77])
+    psf = mvd_synth.generate.random_psf(rng, box)               # asymmetric: a missing mirror fails
+    view = (rng.random((nz, ny, nx), dtype=np.float32) * 100.0 + 5.0)
+    dview = torch.from_numpy(view).cuda()
+    d = mvd.Deconvolver([dview], [psf], variant="osem", kernel_mode="plain")
+    mx, my, mz = d.fft_dims
+    assert mx >= 512 + 24 and my >= 1024 + 12 and mz >= 512 + 25     # M >= N + r (hx + 2 rx along x)
+    pn = O.normalise(psf)
+    cz, cy, cx = [(k - 1) // 2 for k in pn.shape]
+    # sampled voxels: corners, faces, interior
+    pts = [(0, 0, 0), (nz - 1, ny - 1, nx - 1), (0, ny - 1, 5), (nz - 1, 0, nx // 2), (nz // 2, ny // 2, nx // 2 - 1),
+           (nz // 2, ny // 2, nx // 2), (3, 511, 512), (300, 1023, 0)]
+    pts += [tuple(int(rng.integers(n)) for n in (nz, ny, nx)) for _ in range(40)]
+    for which, k in ((0, pn), (1, O.flip(pn))):
+        got = d.convolve(0, which, dview)
+        for (z, y, x) in pts:
+            acc = 0.0                                            # same(a,k)[xi] = sum_u k[u] a[xi - (u - c)]
+            for uz in range(k.shape[0]):
+                zz = z - (uz - cz)
+                if zz < 0 or zz >= nz:
+                    continue
+                y0, y1 = max(0, y + cy - (ny - 1)), min(k.shape[1] - 1, y + cy)
+                x0, x1 = max(0, x + cx - (nx - 1)), min(k.shape[2] - 1, x + cx)
+                kk = k[uz, y0:y1 + 1, x0:x1 + 1].astype(np.float64)
+                aa = view[zz, y + cy - y1:y + cy - y0 + 1, x + cx - x1:x + cx - x0 + 1].astype(np.float64)[::-1, ::-1]
+                acc += float((kk * aa).sum())
+            gv = float(got[z, y, x])
+            assert abs(gv - acc) <= 2e-5 * abs(acc), (which, (z, y, x), gv, acc)
+        del got
+    d.iterate(1)
+    st = d.get_stats()
+    d.close()
+    assert st["flux"] == pytest.approx(float(view.astype(np.float64).sum()), rel=2e-6)
