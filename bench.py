@@ -182,6 +182,21 @@ def load_problem(k, rank, world, dist):
     return mvd_synth.Problem(k, rec["dims"], rec["psf"], None, psfs, views, rec["iterations"], rec["variants"])
 
 
+def max_over_ranks(values, world, dist, device):
+    """Element-wise maximum of a list of floats over all ranks (the slowest replica sets the time)."""
+    if world == 1:
+        return [float(v) for v in values]
+    import torch
+    t = torch.tensor([float(v) for v in values], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def replica_throughput(world, units_per_replica_step, steps, ms):
+    """Whole-job value of `world` independent replicas: all units of all ranks over the slowest rank's time."""
+    return world * units_per_replica_step * steps / (ms * 1e-3) / 1e9
+
+
 def cpu_baseline(prob, budget_s=12.0):
     """The oracle as it stands, on this box's host cores: whole view-updates of efficient-OSEM on
     the full volume until `budget_s` seconds are spent (at least one)."""
@@ -286,11 +301,8 @@ def run_ours(args):
     classes = d.profile_read()
     d.profile(False)
 
-    if world > 1:
-        tmax = torch.tensor([ms, ms_plain], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms, ms_plain = float(tmax[0]), float(tmax[1])
-    value = world * nvox * V * args.steps / (ms * 1e-3) / 1e9
+    ms, ms_plain = max_over_ranks([ms, ms_plain], world, dist, "cuda")
+    value = replica_throughput(world, nvox * V, args.steps, ms)
 
     # ---- roofline of the dominant kernel class --------------------------------------------------
     peak, peak_src = hbm_peak()
@@ -340,10 +352,7 @@ def run_ours(args):
             job()
         barrier()
         dt = time.perf_counter() - tw0
-        if world > 1:
-            tt = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            dt = float(tt[0])
+        dt = max_over_ranks([dt], world, dist, "cuda")[0]
         e2e = {"value": world * nvox * V * iters * args.e2e_jobs / dt / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                "step": "one whole job: H2D of the %d views from pinned host memory, mvd_create (PSF upload, "
