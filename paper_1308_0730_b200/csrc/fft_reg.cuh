@@ -85,13 +85,73 @@ MVD_CE cdouble ce_root(long long k, long long n) {   // exp(+2*pi*i*k/n)
 // ---------------------------------------------------------------------------------------
 // complex helpers
 // ---------------------------------------------------------------------------------------
+#if defined(MVD_HOST_TEST) || defined(MVD_NO_F32X2)
 MVD_DEV float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 MVD_DEV float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+// a + c * s, c real
+MVD_DEV float2 caxpy(float c, float2 s, float2 a) { return make_float2(MVD_FMA(c, s.x, a.x), MVD_FMA(c, s.y, a.y)); }
+MVD_DEV float2 cscale(float c, float2 s) { return make_float2(c * s.x, c * s.y); }
+MVD_DEV float2 fma2(float ax, float ay, float bx, float by, float cx, float cy) {
+  return make_float2(MVD_FMA(ax, bx, cx), MVD_FMA(ay, by, cy));
+}
+MVD_DEV float2 mul2(float ax, float ay, float bx, float by) { return make_float2(MVD_MUL(ax, bx), MVD_MUL(ay, by)); }
+#else
+// sm_100a packed fp32: one FADD2 / FFMA2 / FMUL2 handles the real and the imaginary part together
+// (IEEE per lane, so results equal the scalar forms bit for bit); halves the issue slots of the
+// butterflies, which is what the x pass is short of.
+// (ax,ay) * (bx,by) + (cx,cy) and (ax,ay) * (bx,by): the operands may repeat or swap the halves of a
+// register pair (SASS operand modes .F32 broadcast, .F32x2.LO_HI swap), so neither costs a move
+MVD_DEV float2 fma2(float ax, float ay, float bx, float by, float cx, float cy) {
+  float2 r;
+  asm("{.reg .b64 ra, rb, rc, rd; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; mov.b64 rc, {%6,%7}; fma.rn.f32x2 rd, ra, rb, rc; mov.b64 {%0,%1}, rd;}"
+      : "=f"(r.x), "=f"(r.y) : "f"(ax), "f"(ay), "f"(bx), "f"(by), "f"(cx), "f"(cy));
+  return r;
+}
+MVD_DEV float2 mul2(float ax, float ay, float bx, float by) {
+  float2 r;
+  asm("{.reg .b64 ra, rb, rd; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; mul.rn.f32x2 rd, ra, rb; mov.b64 {%0,%1}, rd;}"
+      : "=f"(r.x), "=f"(r.y) : "f"(ax), "f"(ay), "f"(bx), "f"(by));
+  return r;
+}
+MVD_DEV float2 cadd(float2 a, float2 b) {
+  float2 r;
+  asm("{.reg .b64 ra, rb, rc; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; add.rn.f32x2 rc, ra, rb; mov.b64 {%0,%1}, rc;}"
+      : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+  return r;
+}
+MVD_DEV float2 csub(float2 a, float2 b) {
+  float2 r;
+  asm("{.reg .b64 ra, rb, rc; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; sub.rn.f32x2 rc, ra, rb; mov.b64 {%0,%1}, rc;}"
+      : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+  return r;
+}
+MVD_DEV float2 caxpy(float c, float2 s, float2 a) {   // a + c * s, c real
+  float2 r;
+  asm("{.reg .b64 rs, rc, ra, rd; mov.b64 rs, {%2,%3}; mov.b64 rc, {%4,%4}; mov.b64 ra, {%5,%6}; fma.rn.f32x2 rd, rs, rc, ra; mov.b64 {%0,%1}, rd;}"
+      : "=f"(r.x), "=f"(r.y) : "f"(s.x), "f"(s.y), "f"(c), "f"(a.x), "f"(a.y));
+  return r;
+}
+MVD_DEV float2 cscale(float c, float2 s) {
+  float2 r;
+  asm("{.reg .b64 rs, rc, rd; mov.b64 rs, {%2,%3}; mov.b64 rc, {%4,%4}; mul.rn.f32x2 rd, rs, rc; mov.b64 {%0,%1}, rd;}"
+      : "=f"(r.x), "=f"(r.y) : "f"(s.x), "f"(s.y), "f"(c));
+  return r;
+}
+#endif
+// a * b and a * conj(b) as  a.x * (b.x, +-b.y) + a.y * (-+b.y, b.x): two packed instructions and one
+// sign flip; the order of operations is fixed, so every kernel rounds a product the same way
 MVD_DEV float2 cmul(float2 a, float2 b) {
-  return make_float2(MVD_FMA(a.x, b.x, -MVD_MUL(a.y, b.y)), MVD_FMA(a.x, b.y, MVD_MUL(a.y, b.x)));
+  const float2 t = mul2(a.x, a.x, b.x, b.y);
+  return fma2(a.y, a.y, -b.y, b.x, t.x, t.y);
 }
 MVD_DEV float2 cmul_conj(float2 a, float2 b) {   // a * conj(b)
-  return make_float2(MVD_FMA(a.x, b.x, MVD_MUL(a.y, b.y)), MVD_FMA(a.y, b.x, -MVD_MUL(a.x, b.y)));
+  const float2 t = mul2(a.y, a.y, b.y, b.x);
+  return fma2(a.x, a.x, b.x, -b.y, t.x, t.y);
+}
+// a * w for a table entry e = (w.x, w.y, -w.y, w.x): two packed instructions, no sign flip
+MVD_DEV float2 cmul_tab(float2 a, float4 e) {
+  const float2 t = mul2(a.x, a.x, e.x, e.y);
+  return fma2(a.y, a.y, e.z, e.w, t.x, t.y);
 }
 
 // multiply by exp(DIR * 2*pi*i * K / N), K and N compile-time (DIR = -1 forward, +1 inverse)
@@ -110,7 +170,8 @@ MVD_DEV float2 cmul_root(float2 a) {
     constexpr cdouble w = ce_root(k, N);
     constexpr float c = float(w.re);
     constexpr float s = float(DIR > 0 ? w.im : -w.im);
-    return make_float2(MVD_FMA(a.x, c, -MVD_MUL(a.y, s)), MVD_FMA(a.x, s, MVD_MUL(a.y, c)));
+    const float2 t = mul2(a.x, a.x, c, s);
+    return fma2(a.y, a.y, -s, c, t.x, t.y);
   }
 }
 
@@ -128,12 +189,16 @@ template <int DIR>
 MVD_DEV void bfly4(float2& a, float2& b, float2& c, float2& d) {
   float2 s0 = cadd(a, c), d0 = csub(a, c);
   float2 s1 = cadd(b, d), d1 = csub(b, d);
-  // DIR*i*d1
-  float2 r = DIR > 0 ? make_float2(-d1.y, d1.x) : make_float2(d1.y, -d1.x);
   a = cadd(s0, s1);
   c = csub(s0, s1);
-  b = cadd(d0, r);
-  d = csub(d0, r);
+  // b = d0 + DIR*i*d1, d = d0 - DIR*i*d1 with i*d1 = (-d1.y, d1.x)
+  if constexpr (DIR > 0) {
+    b = make_float2(d0.x - d1.y, d0.y + d1.x);
+    d = make_float2(d0.x + d1.y, d0.y - d1.x);
+  } else {
+    b = make_float2(d0.x + d1.y, d0.y - d1.x);
+    d = make_float2(d0.x - d1.y, d0.y + d1.x);
+  }
 }
 
 // odd prime P: pairs (m, P-m).  X_j = a_j + i*DIR*b_j, X_{P-j} = a_j - i*DIR*b_j with
@@ -158,15 +223,18 @@ MVD_DEV void bfly_odd(float2 (&x)[P]) {
       constexpr int m = decltype(m_)::value + 1;
       constexpr cdouble w = ce_root((long long)j * m, P);
       constexpr float c = float(w.re), sn = float(w.im);
-      a.x += c * s[m - 1].x;
-      a.y += c * s[m - 1].y;
-      b.x += sn * d[m - 1].x;
-      b.y += sn * d[m - 1].y;
+      a = caxpy(c, s[m - 1], a);
+      if constexpr (m == 1) b = cscale(sn, d[0]);
+      else b = caxpy(sn, d[m - 1], b);
     });
-    // i*DIR*b = DIR * (-b.y, b.x)
-    float2 ib = DIR > 0 ? make_float2(-b.y, b.x) : make_float2(b.y, -b.x);
-    x[j] = cadd(a, ib);
-    x[P - j] = csub(a, ib);
+    // x[j] = a + i*DIR*b, x[P-j] = a - i*DIR*b with i*b = (-b.y, b.x)
+    if constexpr (DIR > 0) {
+      x[j] = make_float2(a.x - b.y, a.y + b.x);
+      x[P - j] = make_float2(a.x + b.y, a.y - b.x);
+    } else {
+      x[j] = make_float2(a.x + b.y, a.y - b.x);
+      x[P - j] = make_float2(a.x - b.y, a.y + b.x);
+    }
   });
 }
 
