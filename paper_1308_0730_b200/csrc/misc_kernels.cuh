@@ -109,31 +109,41 @@ __global__ void __launch_bounds__(128) autocorr_kernel(const double* __restrict_
 
 // kern[j] *= sum_u flipPv[u] G[off + j - u],  flipPv[u] = Pv[K-1-u], off = (Gd-1)/2, j in the box of
 // P_v: the central crop of the full convolution P_v* (*) G (R6).  G = P_w (*) P_w* (eq. 105) or P_w (eq. 107).
-// One warp per output tap: the lanes share the (uz, uy) rows of the sum, then a shuffle reduction.
-__global__ void __launch_bounds__(128) corr_crop_mul_kernel(const double* __restrict__ Pv, Dims3 K,
+// One block per 32 consecutive output taps (lane = tap: the G reads of a warp are contiguous, the Pv
+// read is a broadcast); the 8 warps of the block share the (uz, uy) rows of the sum and are reduced
+// through shared memory.
+__global__ void __launch_bounds__(256) corr_crop_mul_kernel(const double* __restrict__ Pv, Dims3 K,
                                                             const double* __restrict__ G, Dims3 Gd,
                                                             double* __restrict__ kern) {
+  __shared__ double red[8][32];
   const long long tot = (long long)K.x * K.y * K.z;
-  const long long j = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;   // warp-uniform
-  if (j >= tot) return;
-  const int lane = threadIdx.x & 31;
-  const int jx = int(j % K.x), jy = int((j / K.x) % K.y), jz = int(j / ((long long)K.x * K.y));
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long j = (long long)blockIdx.x * 32 + lane;
+  const bool live = j < tot;
+  const long long jj = live ? j : tot - 1;
+  const int jx = int(jj % K.x), jy = int((jj / K.x) % K.y), jz = int(jj / ((long long)K.x * K.y));
   const int ox = (Gd.x - 1) / 2 + jx, oy = (Gd.y - 1) / 2 + jy, oz = (Gd.z - 1) / 2 + jz;
-  // g index = o - u in [0, Gd)  ->  u in (o - Gd, o]
-  const int uz0 = max(0, oz - Gd.z + 1), uz1 = min(K.z - 1, oz);
-  const int uy0 = max(0, oy - Gd.y + 1), uy1 = min(K.y - 1, oy);
-  const int ux0 = max(0, ox - Gd.x + 1), ux1 = min(K.x - 1, ox);
-  const int nyr = uy1 - uy0 + 1;
-  const int nrows = (uz1 - uz0 + 1) * nyr;
   double acc = 0.0;
-  for (int r = lane; r < nrows; r += 32) {
-    const int uz = uz0 + r / nyr, uy = uy0 + r % nyr;
+  const int nrows = K.z * K.y;
+  for (int r = warp; r < nrows; r += 8) {
+    const int uz = r / K.y, uy = r - uz * K.y;
+    const int gz = oz - uz, gy = oy - uy;                      // g index = o - u must lie in [0, Gd)
+    if (gz < 0 || gz >= Gd.z || gy < 0 || gy >= Gd.y) continue;
     const double* pv = Pv + ((long long)(K.z - 1 - uz) * K.y + (K.y - 1 - uy)) * K.x;
-    const double* g = G + ((long long)(oz - uz) * Gd.y + (oy - uy)) * Gd.x;
-    for (int ux = ux0; ux <= ux1; ++ux) acc += pv[K.x - 1 - ux] * g[ox - ux];
+    const double* g = G + ((long long)gz * Gd.y + gy) * Gd.x;
+    for (int ux = 0; ux < K.x; ++ux) {
+      const int gx = ox - ux;
+      if (gx >= 0 && gx < Gd.x) acc += pv[K.x - 1 - ux] * g[gx];
+    }
   }
-  acc = warp_sum(acc);
-  if (lane == 0) kern[j] *= acc;
+  red[warp][lane] = acc;
+  __syncthreads();
+  if (warp == 0 && live) {
+    double s = 0.0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) s += red[w][lane];
+    kern[j] *= s;
+  }
 }
 
 // kern[j] = (P[K-1-j])^power  (mirror, L312; power = V gives eq. 108, R9)

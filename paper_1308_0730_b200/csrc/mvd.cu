@@ -745,7 +745,7 @@ mvd_status precompute(mvd_ctx* c, const float* const* psfs_host) {
   for (int v = 0; v < P.V; ++v) {
     const Dims3 K = P.K[v];
     const long long tot = (long long)K.x * K.y * K.z;
-    const unsigned g256 = (unsigned)((tot + 255) / 256), g128 = (unsigned)((tot + 3) / 4);   // corr: one warp per tap
+    const unsigned g256 = (unsigned)((tot + 255) / 256), g128 = (unsigned)((tot + 31) / 32);   // corr: one block of 256 threads per 32 taps
     flip_pow_kernel<<<g256, 256, 0, c->stream>>>(c->psf(v), K, P.kmode == MVD_KERNEL_OPT2 ? P.V : 1, c->kern(v));
     MVD_CK(cudaGetLastError(), "flip_pow_kernel");
     ++c->launches;
@@ -754,10 +754,10 @@ mvd_status precompute(mvd_ctx* c, const float* const* psfs_host) {
         if (w == v) continue;
         const Dims3 Kw = P.K[w];
         if (P.kmode == MVD_KERNEL_COMPOUND)
-          corr_crop_mul_kernel<<<g128, 128, 0, c->stream>>>(c->psf(v), K, c->autoc(w),
+          corr_crop_mul_kernel<<<g128, 256, 0, c->stream>>>(c->psf(v), K, c->autoc(w),
                                                             Dims3{2 * Kw.x - 1, 2 * Kw.y - 1, 2 * Kw.z - 1}, c->kern(v));
         else
-          corr_crop_mul_kernel<<<g128, 128, 0, c->stream>>>(c->psf(v), K, c->psf(w), Kw, c->kern(v));
+          corr_crop_mul_kernel<<<g128, 256, 0, c->stream>>>(c->psf(v), K, c->psf(w), Kw, c->kern(v));
         MVD_CK(cudaGetLastError(), "corr_crop_mul_kernel");
         ++c->launches;
       }
