@@ -577,7 +577,7 @@ mvd_status x_pass(mvd_ctx* c, const XArgs& a_in, int mode) {
   static const int cls[4] = {MVD_K_X_LOAD, MVD_K_X_QUOT, MVD_K_X_UPDATE, MVD_K_X_ACCUM};
   const Plan& P = c->P;
   XArgs a = a_in;
-  const bool tma = P.xtma && (mode == X_QUOT || mode == X_UPDATE);
+  const bool tma = P.xtma && (mode == X_QUOT || mode == X_UPDATE || (mode == X_ACCUM && a_in.acc_mode != ACC_STORE));
   if (tma) {
     // persistent CTAs, tiles of Rxt rows staged by bulk copies (pass_tma.cuh)
     a.rows_per_cta = P.Rxt;
@@ -585,7 +585,7 @@ mvd_status x_pass(mvd_ctx* c, const XArgs& a_in, int mode) {
     a.real_stride = P.xt_rstride;
     a.reverse = c->use_flip ? (c->flip ^= 1) : 0;
     a.exch_stride = P.xt_exch; a.exch_stride_g = P.xt_exch_g; a.exch_stride_f = P.xt_exch_f;
-    const float* real_src = mode == X_QUOT ? a.phi : a.psi;
+    const float* real_src = mode == X_QUOT ? a.phi : (mode == X_UPDATE ? a.psi : a.acc);
     a.bulk_real = (P.N[0] % 4 == 0) && ((reinterpret_cast<size_t>(real_src) & 15) == 0);
     if (c->xt_blocks[mode] == 0) {
       c->xt_blocks[mode] = P.lx->xrow_tma_blocks_per_sm(mode, a.nthreads, P.lx->xrow_tma_smem(a.rows_per_cta, P.r[0], P.N[0]));

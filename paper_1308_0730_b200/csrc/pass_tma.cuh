@@ -42,7 +42,14 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
   using Cfg = PassCfg<A, B>;
   constexpr int M = Cfg::M, AP = Cfg::AP, BP = Cfg::BP;
   constexpr int CS = xrow_cstride(M, A);
-  static_assert(MODE == X_QUOT || MODE == X_UPDATE, "TMA-staged x pass: quotient and OSEM update only");
+  static_assert(MODE == X_QUOT || MODE == X_UPDATE || MODE == X_ACCUM, "TMA-staged x pass: no X_LOAD");
+  // X_ACCUM (combined variants): running product of the f_v in acc; the last view takes the root,
+  // updates psi and transforms the new estimate.  acc is the staged real row (read for MID / LAST).
+  const bool acc_read = MODE == X_ACCUM && (p.acc_mode == ACC_MID || p.acc_mode == ACC_LAST);
+  const bool acc_last = MODE == X_ACCUM && (p.acc_mode == ACC_LAST || p.acc_mode == ACC_ONLY);
+  const bool do_forward = MODE != X_ACCUM || acc_last;
+  const bool need_real = MODE != X_ACCUM || acc_read;          // real rows staged at all
+  const bool real_bulk = need_real && p.bulk_real, real_plain = need_real && !p.bulk_real;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int R = p.rows_per_cta;
   const int RSTR = p.real_stride;
@@ -59,7 +66,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
   uint64_t* bars = reinterpret_cast<uint64_t*>(
       (reinterpret_cast<uintptr_t>(halo_im + R * p.rx) + 7) & ~uintptr_t(7));
   const int tid = threadIdx.x;
-  const float* real_src = MODE == X_QUOT ? p.phi : p.psi;
+  const float* real_src = MODE == X_QUOT ? p.phi : (MODE == X_UPDATE ? p.psi : p.acc);
   const int ntiles = (int)((p.nrows + R - 1) / R);
   const int nrows_i = (int)p.nrows;
 
@@ -100,7 +107,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
 
   if (tid < 32 && (int)blockIdx.x < ntiles) {
     issue_w((int)blockIdx.x);
-    if (p.bulk_real) issue_r((int)blockIdx.x);
+    if (real_bulk) issue_r((int)blockIdx.x);
   }
 
   int it = 0;
@@ -110,7 +117,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
     const bool actA = tid < R * A && growA < nrows_i;
     const bool actB = tid < R * B && growB < nrows_i;
     const bool more = tile + (int)gridDim.x < ntiles;
-    if (!p.bulk_real) {   // rows not 16-byte aligned: plain loads of this tile's real rows
+    if (real_plain) {   // rows not 16-byte aligned: plain loads of this tile's real rows
       const int rv = min(R, nrows_i - row0);
       for (int i = tid; i < rv * p.nx; i += blockDim.x) {
         const int r = i / p.nx, x = i - r * p.nx;
@@ -157,70 +164,73 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
       });
     }
     __syncthreads();
-    if (p.bulk_real) mbar_wait(&bars[1], it & 1);
+    if (real_bulk) mbar_wait(&bars[1], it & 1);
     // ---- pointwise stage on the real row -------------------------------------------------------
     if (actB) {
       const long long rbase = (long long)growB * p.nx;
       const float* rrow = rst + (size_t)rowB * RSTR;
       float* prow = p.psi + rbase;
+      float* arow = p.acc + rbase;
       const int lo_int = p.rx, hi_int = min(p.hx - p.rx, p.nx - p.hx);   // interior: no overlap, both halves live
+      // one voxel: x = row position, v = convolution result there; returns the value carried into
+      // the forward transform (quotient / new estimate / nothing)
+      auto voxel = [&](int x, float v) -> float {
+        if constexpr (MODE == X_QUOT) {
+          return __fdividef(rrow[x], fmaxf(v, p.eps));                    // S2, R4
+        } else if constexpr (MODE == X_UPDATE) {
+          const float o = rrow[x];
+          const float nw = fmaxf(o * v, p.psi_floor);                     // eq. 109-112, R4
+          prow[x] = nw;
+          flux += nw;
+          l1 += fabsf(nw - o);
+          return nw;
+        } else {                                                          // X_ACCUM (eq. 70 / 104, R1)
+          float f = p.literal_product ? v : fmaxf(v, 0.f);
+          if (acc_read) f *= rrow[x];
+          if (!acc_last) {
+            arow[x] = f;
+            return 0.f;
+          }
+          if (!p.literal_product && p.inv_nviews != 1.f) f = powf(f, p.inv_nviews);
+          const float o = prow[x];
+          const float nw = fmaxf(o * f, p.psi_floor);
+          prow[x] = nw;
+          flux += nw;
+          l1 += fabsf(nw - o);
+          return nw;
+        }
+      };
       static_for<0, A>([&](auto n1_) {
         constexpr int n1 = decltype(n1_)::value;
         const int n = n1 * B + n2;
         float2 z = make_float2(0.f, 0.f);
         if (n1 * B >= lo_int && n1 * B + B <= hi_int) {     // warp-uniform fast path
-          if constexpr (MODE == X_QUOT) {
-            z.x = __fdividef(rrow[n], fmaxf(c[n1].x, p.eps));
-            z.y = __fdividef(rrow[n + p.hx], fmaxf(c[n1].y, p.eps));
-          } else {
-            const float o = rrow[n], o2 = rrow[n + p.hx];
-            const float nw = fmaxf(o * c[n1].x, p.psi_floor), nw2 = fmaxf(o2 * c[n1].y, p.psi_floor);
-            prow[n] = nw;
-            prow[n + p.hx] = nw2;
-            flux += nw + nw2;
-            l1 += fabsf(nw - o) + fabsf(nw2 - o2);
-            z = make_float2(nw, nw2);
-          }
+          z.x = voxel(n, c[n1].x);
+          z.y = voxel(n + p.hx, c[n1].y);
         } else if (n < p.hx) {
           float vt = c[n1].x, vb = c[n1].y;
           if (n >= p.hx - p.rx) vt += halo_im[rowB * p.rx + (n - (p.hx - p.rx))];
           if (n < p.rx) vb += halo_re[rowB * p.rx + n];
-          const bool has_b = n + p.hx < p.nx;
-          if constexpr (MODE == X_QUOT) {
-            z.x = __fdividef(rrow[n], fmaxf(vt, p.eps));
-            if (has_b) z.y = __fdividef(rrow[n + p.hx], fmaxf(vb, p.eps));
-          } else {
-            const float o = rrow[n];
-            const float nw = fmaxf(o * vt, p.psi_floor);
-            p.psi[rbase + n] = nw;
-            flux += nw;
-            l1 += fabsf(nw - o);
-            z.x = nw;
-            if (has_b) {
-              const float o2 = rrow[n + p.hx];
-              const float nw2 = fmaxf(o2 * vb, p.psi_floor);
-              p.psi[rbase + n + p.hx] = nw2;
-              flux += nw2;
-              l1 += fabsf(nw2 - o2);
-              z.y = nw2;
-            }
-          }
+          z.x = voxel(n, vt);
+          if (n + p.hx < p.nx) z.y = voxel(n + p.hx, vb);
         }
         c[n1] = z;
       });
       // ---- F1: forward A-point transforms over n1 ----------------------------------------------
-      FftReg<A, -1>::run(c);
-      static_for<0, A>([&](auto k1_) {
-        constexpr int kk = decltype(k1_)::value;
-        if constexpr (kk > 0) c[kk] = cmul(c[kk], tw2[n2 * AP + kk]);
-        sm[rowB * RSF + kk * BP + n2] = c[kk];
-      });
+      if (do_forward) {
+        FftReg<A, -1>::run(c);
+        static_for<0, A>([&](auto k1_) {
+          constexpr int kk = decltype(k1_)::value;
+          if constexpr (kk > 0) c[kk] = cmul(c[kk], tw2[n2 * AP + kk]);
+          sm[rowB * RSF + kk * BP + n2] = c[kk];
+        });
+      }
     }
     __syncthreads();
     // every read of the real rows is done: stage the next tile's
-    if (tid < 32 && more && p.bulk_real) issue_r(tile + (int)gridDim.x);
+    if (tid < 32 && more && real_bulk) issue_r(tile + (int)gridDim.x);
     // ---- F2: forward B-point transforms over n2, store k = k1 + A*k2 ---------------------------
-    if (actA) {
+    if (actA && do_forward) {
       float2 u[B];
       static_for<0, B>([&](auto n2_) {
         constexpr int m = decltype(n2_)::value;
@@ -240,7 +250,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArg
   }
 
   // ---- per-CTA statistics of the update: {sum psi_new, sum |psi_new - psi_old|} ----------------
-  if constexpr (MODE == X_UPDATE) {
+  if (MODE == X_UPDATE || acc_last) {
     double df = dflux, dl = dl1;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -518,6 +528,7 @@ struct LaunchTma {
   if (e != cudaSuccess) { fprintf(stderr, "carveout attr failed %d x %d: %s\n", A, B, #k); return e; }
     MVD_SET((xrow_tma_kernel<A, B, X_QUOT>));
     MVD_SET((xrow_tma_kernel<A, B, X_UPDATE>));
+    MVD_SET((xrow_tma_kernel<A, B, X_ACCUM>));
     MVD_SET((strided_tma_kernel<A, B, -1>));
     MVD_SET((strided_tma_kernel<A, B, 1>));
     MVD_SET((zconv_tma_kernel<A, B>));
@@ -529,7 +540,9 @@ struct LaunchTma {
     int n = 0;
     cudaError_t e = mode == X_QUOT
         ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_QUOT>, nthreads, smem)
-        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_UPDATE>, nthreads, smem);
+        : mode == X_UPDATE
+        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_UPDATE>, nthreads, smem)
+        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_ACCUM>, nthreads, smem);
     return e == cudaSuccess ? n : 0;
   }
 
@@ -569,6 +582,7 @@ struct LaunchTma {
     const size_t smem = xrow_smem(a.rows_per_cta, a.rx, a.nx);
     if (mode == X_QUOT) xrow_tma_kernel<A, B, X_QUOT><<<a.grid, a.nthreads, smem, s>>>(a);
     else if (mode == X_UPDATE) xrow_tma_kernel<A, B, X_UPDATE><<<a.grid, a.nthreads, smem, s>>>(a);
+    else if (mode == X_ACCUM) xrow_tma_kernel<A, B, X_ACCUM><<<a.grid, a.nthreads, smem, s>>>(a);
     else return cudaErrorInvalidValue;
     return cudaGetLastError();
   }
