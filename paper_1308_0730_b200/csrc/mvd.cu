@@ -260,12 +260,12 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
       // two tile stages whenever they fit (one stage with more CTAs per SM measured slower on config 5)
       const int nbox = (P.ly->M + 255) / 256;
       const int boxr = ((P.ly->M + nbox - 1) / nbox + 3) / 4 * 4;
-      P.ynst = P.ly->strided_tma_smem(kTmaTileHost, boxr, nbox, 2) <= 200 * 1024 ? 2 : 1;
+      P.ynst = P.ly->strided_tma_smem(kTmaTileHost, boxr, nbox, 2) <= 218 * 1024 ? 2 : 1;
       const int force = env_int("MVD_YNST", 0);
       if (force == 1 || force == 2) P.ynst = force;
       const int nbz = (P.lz->M + 255) / 256;
       const int bxz = ((P.lz->M + nbz - 1) / nbz + 3) / 4 * 4;
-      if (env_int("MVD_ZNST", 0) == 0) P.znst = P.lz->zconv_tma_smem(kTmaTileHost, bxz, nbz, 2) <= 200 * 1024 ? 2 : 1;
+      if (env_int("MVD_ZNST", 0) == 0) P.znst = P.lz->zconv_tma_smem(kTmaTileHost, bxz, nbz, 2) <= 218 * 1024 ? 2 : 1;
     }
     P.ytma = env_int("MVD_YTMA", 1);
     P.ztma = env_int("MVD_ZTMA", 1);
@@ -278,7 +278,8 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
     P.xtma = env_int("MVD_XTMA", 1);
     int R = std::max(1, 160 / ab);   // kXrowTmaThreads of pass_tma.cuh
     const int force = env_int("MVD_RXT", 0);
-    const size_t cap = (size_t)env_int("MVD_XT_SMEM_KB", 45) * 1024;
+    // 45 KB: five CTAs per SM; larger radices hold fewer CTAs (registers), so they get larger tiles
+    const size_t cap = (size_t)env_int("MVD_XT_SMEM_KB", ab <= 21 ? 45 : (ab <= 28 ? 72 : 100)) * 1024;
     while (R > 1 && P.lx->xrow_tma_smem(R, P.r[0], P.N[0]) > cap) --R;
     if (force > 0 && force * ab <= 160 && P.lx->xrow_tma_smem(force, P.r[0], P.N[0]) <= 220 * 1024) R = force;
     if (P.lx->xrow_tma_smem(R, P.r[0], P.N[0]) > 220 * 1024) P.xtma = 0;

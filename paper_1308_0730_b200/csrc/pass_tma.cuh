@@ -34,11 +34,13 @@ __host__ __device__ constexpr int xrow_rstride(int nx, int B) {
 // tile width (contiguous complex elements) of the TMA-staged y and z passes: compile-time, so every
 // shared-memory offset of the in-place transforms is an immediate
 constexpr int kTmaTile = kTmaTileHost;
-// thread cap of the TMA-staged x pass: 4+ resident CTAs per SM at <= 102 registers per thread
+// thread cap of the TMA-staged x pass, and the resident CTAs per SM its register budget is sized for:
+// 4 (<= 102 registers) while the larger transform has <= 21 points, fewer for larger radices (no spills)
 constexpr int kXrowTmaThreads = 160;
+constexpr int xrow_min_blocks(int ab_max) { return ab_max <= 21 ? 4 : (ab_max <= 28 ? 3 : 2); }
 
 template <int A, int B, int MODE>
-__global__ void __launch_bounds__(kXrowTmaThreads, 4) xrow_tma_kernel(const XArgs p) {
+__global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>::AB_MAX)) xrow_tma_kernel(const XArgs p) {
   using Cfg = PassCfg<A, B>;
   constexpr int M = Cfg::M, AP = Cfg::AP, BP = Cfg::BP;
   constexpr int CS = xrow_cstride(M, A);

@@ -374,3 +374,17 @@ def test_config5_size_sampled_voxels_and_flux(mvd):
     st = d.get_stats()
     d.close()
     assert st["flux"] == pytest.approx(float(view.astype(np.float64).sum()), rel=2e-6)
+
+
+def test_repeated_runs_are_bit_identical(mvd, config2):
+    """The staged pipelines (mbarrier phases, refilled tiles) must not race: the same problem run
+    several times in fresh contexts, with plain launches and under graph replay, gives the same bits."""
+    ref = None
+    for rep in range(4):
+        g, _ = gpu_checkpoints(mvd, config2, "osem", "auto", (3,), use_graph=bool(rep & 1))
+        if ref is None:
+            ref = g[3]
+        assert np.array_equal(g[3], ref), "run %d differs" % rep
+    g, _ = gpu_checkpoints(mvd, config2, "efficient", "auto", (2,))
+    h, _ = gpu_checkpoints(mvd, config2, "efficient", "auto", (2,))
+    assert np.array_equal(g[2], h[2])
