@@ -88,6 +88,12 @@ typedef struct {
   size_t workspace_bytes;
   void* stream;              /* cudaStream_t                                                */
   int use_graph;             /* 1: mvd_iterate replays one captured CUDA graph per iteration (needs a non-default stream: MVD_ERR_UNSUPPORTED otherwise) */
+  const float* const* weights; /* optional: n_views DEVICE pointers to per-view weight images (N voxels each, values in
+                                * [0,1], borrowed like the views), section 12: a sequential update
+                                * applies the fraction w_v of the change an RL step suggests,
+                                * psi <- max(psi * (1 + w_v (f_v - 1)), floor).  MVD_OSEM only (else
+                                * MVD_ERR_UNSUPPORTED).  NULL -> no weights.  How the weights are built (cosine
+                                * blending, sum over views <= c) is the caller's business. */
 } mvd_options;
 
 /* Fills *opt with the defaults (struct_size set, everything else 0/NULL/defaults). */

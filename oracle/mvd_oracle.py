@@ -194,9 +194,11 @@ class Oracle:
     """
 
     def __init__(self, views, psfs, variant="osem", kernel_mode="auto", literal_product=False,
-                 eps=EPS_DEFAULT, psi_floor=FLOOR_DEFAULT, psi0=None, backend="fft"):
+                 eps=EPS_DEFAULT, psi_floor=FLOOR_DEFAULT, psi0=None, backend="fft", weights=None):
         if variant not in VARIANTS:
             raise ValueError(variant)
+        if weights is not None and variant != "osem":
+            raise ValueError("per-view weights belong to the sequential updates (section 12, L897)")
         if kernel_mode not in KERNEL_MODES:
             raise ValueError(kernel_mode)
         self.views = [np.asarray(v, dtype=np.float64) for v in views]
@@ -212,6 +214,7 @@ class Oracle:
         self.backend = backend
         self.kernels = [back_projector(self.psfs, v, self.kernel_mode, backend)
                         for v in range(len(self.psfs))]
+        self.weights = None if weights is None else [np.asarray(w, dtype=np.float64) for w in weights]
         self.psi = initial_estimate(self.views) if psi0 is None else np.array(psi0, dtype=np.float64)
         self.iterations_done = 0
         self.flux = float(self.psi.sum())
@@ -232,7 +235,13 @@ class Oracle:
             if self.variant == "osem":
                 # eq. 109-112 / 114-117: psi is updated after every view, index order (R11)
                 for v in range(nv):
-                    self._commit(np.maximum(self.psi * self.factor(v), self.psi_floor))
+                    f = self.factor(v)
+                    if self.weights is not None:
+                        # section 12 (L897): the weight 0..1 of a pixel is "the fraction of change
+                        # suggested by a Lucy-Richardson update step that will be applied":
+                        # psi*f = psi + (psi*f - psi)  ->  psi + w*(psi*f - psi) = psi*(1 + w*(f - 1))
+                        f = 1.0 + self.weights[v] * (f - 1.0)
+                    self._commit(np.maximum(self.psi * f, self.psi_floor))
             else:
                 # eq. 70 / 104: every f_v from the same psi^r, multiplicative combination
                 prod = np.ones_like(self.psi)
@@ -250,6 +259,36 @@ def deconvolve(views, psfs, variant="osem", iterations=1, **kw):
     o = Oracle(views, psfs, variant, **kw)
     o.iterate(iterations)
     return o.psi
+
+
+# --------------------------------------------------------------------------------------
+# section 12 (L891-903): weight images for partially overlapping views
+# --------------------------------------------------------------------------------------
+def blending_weights(shape_zyx, lo_zyx, hi_zyx, border):
+    """Weight image of one view whose data covers the box [lo, hi) of the common frame: 1 in the
+    central part, falling to 0 at the faces of the box "following a cosine function" over
+    `border` voxels (L891), 0 outside the box.  Per axis the ramp at distance d (in voxels, the
+    face voxel has d = 0.5) is 0.5*(1 - cos(pi*d/border)); the three axes multiply.  [reading R16:
+    the paper gives neither the ramp width nor how axes combine]"""
+    w = np.ones(shape_zyx, dtype=np.float64)
+    for ax in range(3):
+        idx = np.arange(shape_zyx[ax], dtype=np.float64)
+        d = np.minimum(idx - lo_zyx[ax] + 0.5, hi_zyx[ax] - idx - 0.5)     # distance to the nearer face
+        r = np.where(d <= 0, 0.0, np.where(d >= border, 1.0, 0.5 * (1.0 - np.cos(np.pi * d / border))))
+        sh = [1, 1, 1]
+        sh[ax] = -1
+        w = w * r.reshape(sh)
+    return w
+
+
+def normalise_weights(weights, max_sum=1.0):
+    """Scale the weights of every pixel so that their sum over the views is <= max_sum (default 1:
+    "normalized to <= 1", L897; max_sum = number of overlapping views the user allows, L903).
+    Weights are only ever scaled down: "individual weights are never increased above 1" (L895)."""
+    ws = [np.asarray(w, dtype=np.float64) for w in weights]
+    tot = np.sum(ws, axis=0)
+    scale = np.where(tot > max_sum, max_sum / np.maximum(tot, 1e-300), 1.0)
+    return [w * scale for w in ws]
 
 
 # --------------------------------------------------------------------------------------

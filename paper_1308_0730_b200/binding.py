@@ -45,6 +45,7 @@ class mvd_options(C.Structure):
         ("workspace_bytes", C.c_size_t),
         ("stream", C.c_void_p),
         ("use_graph", C.c_int),
+        ("weights", C.c_void_p),
     ]
 
 
@@ -168,7 +169,8 @@ class Deconvolver:
     alive here); ``psfs``: list of host arrays (Kz,Ky,Kx)."""
 
     def __init__(self, views, psfs, variant="osem", kernel_mode="auto", literal_product=False,
-                 eps=None, psi_floor=None, psi0=None, fft_dims=None, use_graph=False, stream=None):
+                 eps=None, psi_floor=None, psi0=None, fft_dims=None, use_graph=False, stream=None,
+                 weights=None):
         import torch
 
         lib = load_library()
@@ -204,6 +206,15 @@ class Deconvolver:
         if psi0 is not None:
             self._psi0 = psi0.to(device=self.device, dtype=torch.float32).contiguous()
             opt.psi0 = self._psi0.data_ptr()
+        self._weights = None
+        if weights is not None:
+            if len(weights) != len(views):
+                raise MvdError("need one weight image per view")
+            self._weights = [w.to(device=self.device, dtype=torch.float32).contiguous() for w in weights]
+            if any(tuple(w.shape) != shape for w in self._weights):
+                raise MvdError("weight images must have the shape of the views")
+            self._weight_ptrs = (C.c_void_p * len(views))(*[w.data_ptr() for w in self._weights])
+            opt.weights = C.cast(self._weight_ptrs, C.c_void_p)
         self.workspace_bytes = int(nbytes)
         view_ptrs = (C.c_void_p * len(views))(*[v.data_ptr() for v in self.views])
         ctx = C.c_void_p()

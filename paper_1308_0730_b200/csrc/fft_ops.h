@@ -81,7 +81,8 @@ enum XMode {
   X_LOAD = 0,              // (psi | complex rows) -> forward FFT
   X_QUOT = 1,              // inverse FFT -> q = phi / max(b, eps) -> forward FFT
   X_UPDATE = 2,            // inverse FFT -> psi <- max(psi*f, floor) -> forward FFT   (OSEM)
-  X_ACCUM = 3              // inverse FFT -> raw store | product accumulation | final combined update
+  X_ACCUM = 3,             // inverse FFT -> raw store | product accumulation | final combined update
+  X_UPDATE_W = 4           // X_UPDATE with a per-view weight image (section 12): psi <- psi*(1 + w (f - 1))
 };
 enum AccMode { ACC_STORE = 0, ACC_FIRST = 1, ACC_MID = 2, ACC_LAST = 3, ACC_ONLY = 4 };
 
@@ -98,6 +99,7 @@ struct XArgs {
   int hx;                  // (Nx+1)/2: element n of the half row carries x=n (re) and x=n+hx (im)
   int rx;                  // PSF half-size along x of this view
   const float* phi;        // X_QUOT: view; X_LOAD: psi (real input)
+  const float* wts;        // X_UPDATE: weight image of this view (section 12) or NULL
   float* psi;              // X_UPDATE / ACC_LAST: estimate, updated in place
   float* acc;              // X_ACCUM: product accumulator / raw destination
   double* partials;        // per-CTA {flux, l1} (X_UPDATE, ACC_LAST)
@@ -126,7 +128,7 @@ struct LengthOps {
   size_t (*xrow_smem)(int rows, int rx);
   // TMA-staged passes (pass_tma.cuh)
   cudaError_t (*xrow_tma)(const XArgs&, int mode, cudaStream_t);
-  size_t (*xrow_tma_smem)(int rows, int rx, int nx);
+  size_t (*xrow_tma_smem)(int rows, int rx, int nx, int weighted);
   int (*xrow_tma_blocks_per_sm)(int mode, int nthreads, size_t smem);
   cudaError_t (*strided_tma)(const StridedTmaArgs&, int dir, cudaStream_t);
   size_t (*strided_tma_smem)(int T, int boxr, int nbox, int nst);

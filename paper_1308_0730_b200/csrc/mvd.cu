@@ -80,6 +80,7 @@ struct Plan {
   int Mx = 0, My = 0, Mz = 0;
   long long nvox = 0, plane = 0, wsize = 0, ssize = 0;   // elements
   bool combined = false;
+  int weighted = 0;              // per-view weight images given (section 12): the x update stages them too
   int kmode = MVD_KERNEL_PLAIN;
   // tiles
   int Ty = 0, nty = 0, Tz = 0, ntz = 0, Tzs = 0, ntzs = 0, Tys = 0, ntys = 0, Rx = 0, ntx = 0;
@@ -176,6 +177,8 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
   P.kmode = kmode;
   P.V = n_views;
   P.combined = variant != MVD_OSEM;
+  P.weighted = (opt && opt->weights) ? 1 : 0;
+  if (P.weighted && P.combined) return MVD_ERR_UNSUPPORTED;   // weights belong to the sequential updates (L897)
   for (int a = 0; a < 3; ++a) {
     if (dims[a] < 1 || dims[a] > (1 << 20)) return MVD_ERR_INVALID_ARG;
     P.N[a] = dims[a];
@@ -280,9 +283,9 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
     const int force = env_int("MVD_RXT", 0);
     // 45 KB: five CTAs per SM; larger radices hold fewer CTAs (registers), so they get larger tiles
     const size_t cap = (size_t)env_int("MVD_XT_SMEM_KB", ab <= 21 ? 45 : (ab <= 28 ? 72 : 100)) * 1024;
-    while (R > 1 && P.lx->xrow_tma_smem(R, P.r[0], P.N[0]) > cap) --R;
-    if (force > 0 && force * ab <= 160 && P.lx->xrow_tma_smem(force, P.r[0], P.N[0]) <= 220 * 1024) R = force;
-    if (P.lx->xrow_tma_smem(R, P.r[0], P.N[0]) > 220 * 1024) P.xtma = 0;
+    while (R > 1 && P.lx->xrow_tma_smem(R, P.r[0], P.N[0], P.weighted) > cap) --R;
+    if (force > 0 && force * ab <= 160 && P.lx->xrow_tma_smem(force, P.r[0], P.N[0], P.weighted) <= 220 * 1024) R = force;
+    if (P.lx->xrow_tma_smem(R, P.r[0], P.N[0], P.weighted) > 220 * 1024) P.xtma = 0;
     P.Rxt = R;
     P.ntxt = round_up32(R * ab);
     int s = (P.N[0] + 3) / 4 * 4;
@@ -341,6 +344,7 @@ struct mvd_ctx {
   cudaStream_t stream = nullptr;
   char* ws = nullptr;
   std::vector<const float*> views;
+  std::vector<const float*> weights;   // empty or one per view (borrowed)
   bool w_valid = false;        // the work buffer holds the x-forward transform of the current psi
   bool broken = false;
   bool stats_valid = false;
@@ -352,7 +356,7 @@ struct mvd_ctx {
   long long graph_launches = 0;
   char err[512] = {0};
   int num_sms = 148;
-  int xt_blocks[4] = {0, 0, 0, 0};   // resident CTAs per SM of the TMA-staged x pass, per mode
+  int xt_blocks[5] = {0, 0, 0, 0, 0};   // resident CTAs per SM of the TMA-staged x pass, per mode
   int flip = 0;                      // tile direction of the next x / y launch (alternates: L2 reuse)
   int use_flip = 1;
   int yt_blocks[2] = {0, 0};         // ... of the TMA-staged y pass (forward, inverse)
@@ -575,10 +579,10 @@ XArgs x_args(mvd_ctx* c, const float2* in, float2* out, int rx) {
 }
 
 mvd_status x_pass(mvd_ctx* c, const XArgs& a_in, int mode) {
-  static const int cls[4] = {MVD_K_X_LOAD, MVD_K_X_QUOT, MVD_K_X_UPDATE, MVD_K_X_ACCUM};
+  static const int cls[5] = {MVD_K_X_LOAD, MVD_K_X_QUOT, MVD_K_X_UPDATE, MVD_K_X_ACCUM, MVD_K_X_UPDATE};
   const Plan& P = c->P;
   XArgs a = a_in;
-  const bool tma = P.xtma && (mode == X_QUOT || mode == X_UPDATE || (mode == X_ACCUM && a_in.acc_mode != ACC_STORE));
+  const bool tma = P.xtma && (mode == X_QUOT || mode == X_UPDATE || mode == X_UPDATE_W || (mode == X_ACCUM && a_in.acc_mode != ACC_STORE));
   if (tma) {
     // persistent CTAs, tiles of Rxt rows staged by bulk copies (pass_tma.cuh)
     a.rows_per_cta = P.Rxt;
@@ -586,25 +590,26 @@ mvd_status x_pass(mvd_ctx* c, const XArgs& a_in, int mode) {
     a.real_stride = P.xt_rstride;
     a.reverse = c->use_flip ? (c->flip ^= 1) : 0;
     a.exch_stride = P.xt_exch; a.exch_stride_g = P.xt_exch_g; a.exch_stride_f = P.xt_exch_f;
-    const float* real_src = mode == X_QUOT ? a.phi : (mode == X_UPDATE ? a.psi : a.acc);
-    a.bulk_real = (P.N[0] % 4 == 0) && ((reinterpret_cast<size_t>(real_src) & 15) == 0);
+    const float* real_src = mode == X_QUOT ? a.phi : (mode == X_ACCUM ? a.acc : a.psi);
+    a.bulk_real = (P.N[0] % 4 == 0) && ((reinterpret_cast<size_t>(real_src) & 15) == 0) &&
+                  ((reinterpret_cast<size_t>(a.wts) & 15) == 0);
     if (c->xt_blocks[mode] == 0) {
-      c->xt_blocks[mode] = P.lx->xrow_tma_blocks_per_sm(mode, a.nthreads, P.lx->xrow_tma_smem(a.rows_per_cta, P.r[0], P.N[0]));
+      c->xt_blocks[mode] = P.lx->xrow_tma_blocks_per_sm(mode, a.nthreads, P.lx->xrow_tma_smem(a.rows_per_cta, P.r[0], P.N[0], mode == X_UPDATE_W));
       if (env_int("MVD_XBLK", 0) > 0) c->xt_blocks[mode] = std::min(c->xt_blocks[mode], env_int("MVD_XBLK", 0));
       if (c->xt_blocks[mode] <= 0) { snprintf(c->err, sizeof(c->err), "x pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
     }
     const long long ntiles = (a.nrows + a.rows_per_cta - 1) / a.rows_per_cta;
     a.grid = (int)std::min<long long>(std::min<long long>(ntiles, (long long)c->num_sms * c->xt_blocks[mode]), P.sum_blocks);
     {
-      ProfScope ps(c, cls[mode & 3]);
+      ProfScope ps(c, cls[mode]);
       MVD_CK(P.lx->xrow_tma(a, mode, c->stream), "x pass (TMA)");
     }
   } else {
-    ProfScope ps(c, cls[mode & 3]);
+    ProfScope ps(c, cls[mode]);
     MVD_CK(P.lx->xrow(a, mode, c->stream), "x pass");
   }
   ++c->launches;
-  if (mode == X_UPDATE || (mode == X_ACCUM && (a.acc_mode == ACC_LAST || a.acc_mode == ACC_ONLY))) {
+  if (mode == X_UPDATE || mode == X_UPDATE_W || (mode == X_ACCUM && (a.acc_mode == ACC_LAST || a.acc_mode == ACC_ONLY))) {
     c->stats_valid = true;
     c->stats_ncta = tma ? a.grid : (int)((a.nrows + a.rows_per_cta - 1) / a.rows_per_cta);
   }
@@ -640,7 +645,8 @@ mvd_status iteration_body(mvd_ctx* c) {
       MVD_TRY(x_pass(c, q, X_QUOT));
       MVD_TRY(conv_core(c, nullptr, c->W(), c->specK(v), false));
       XArgs u = x_args(c, c->W(), c->W(), rx);
-      MVD_TRY(x_pass(c, u, X_UPDATE));
+      u.wts = c->weights.empty() ? nullptr : c->weights[v];
+      MVD_TRY(x_pass(c, u, u.wts ? X_UPDATE_W : X_UPDATE));
     }
   } else {
     // eq. 70 / 104: every f_v from the same psi; the x and y forward passes of psi are shared
@@ -875,6 +881,15 @@ mvd_status mvd_create(mvd_ctx** out, int n_views, const float* const* views, con
     return MVD_ERR_UNSUPPORTED;
   }
   c->views.assign(views, views + n_views);
+  if (opt->weights && !c->P.xtma) {   // only the TMA-staged update applies weights
+    delete c;
+    return MVD_ERR_UNSUPPORTED;
+  }
+  if (opt->weights) {
+    for (int v = 0; v < n_views; ++v)
+      if (!opt->weights[v]) { delete c; return MVD_ERR_INVALID_ARG; }
+    c->weights.assign(opt->weights, opt->weights + n_views);
+  }
 
   cudaError_t e = cudaSuccess;
   {

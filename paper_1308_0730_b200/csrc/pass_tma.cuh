@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
   using Cfg = PassCfg<A, B>;
   constexpr int M = Cfg::M, AP = Cfg::AP, BP = Cfg::BP;
   constexpr int CS = xrow_cstride(M, A);
-  static_assert(MODE == X_QUOT || MODE == X_UPDATE || MODE == X_ACCUM, "TMA-staged x pass: no X_LOAD");
+  static_assert(MODE == X_QUOT || MODE == X_UPDATE || MODE == X_UPDATE_W || MODE == X_ACCUM, "TMA-staged x pass: no X_LOAD");
   // X_ACCUM (combined variants): running product of the f_v in acc; the last view takes the root,
   // updates psi and transforms the new estimate.  acc is the staged real row (read for MID / LAST).
   const bool acc_read = MODE == X_ACCUM && (p.acc_mode == ACC_MID || p.acc_mode == ACC_LAST);
@@ -61,14 +61,16 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
   //         next tile as soon as its last reader of this tile has passed a barrier.
   float2* wst = reinterpret_cast<float2*>(smem_raw);
   float* rst = reinterpret_cast<float*>(wst + (size_t)R * CS);
-  float2* sm = reinterpret_cast<float2*>(rst + (size_t)R * RSTR);
+  constexpr bool has_w = MODE == X_UPDATE_W;                      // section 12 weights
+  float* wrst = rst + (size_t)R * RSTR;                           // [R][RSTR] weight rows (only with weights)
+  float2* sm = reinterpret_cast<float2*>(rst + (size_t)(has_w ? 2 : 1) * R * RSTR);
   float2* tw2 = sm + (size_t)R * RS;                              // tw2[n2*AP + k1] = W_M^(n2 k1)
   float* halo_re = reinterpret_cast<float*>(tw2 + B * AP);
   float* halo_im = halo_re + R * p.rx;
   uint64_t* bars = reinterpret_cast<uint64_t*>(
       (reinterpret_cast<uintptr_t>(halo_im + R * p.rx) + 7) & ~uintptr_t(7));
   const int tid = threadIdx.x;
-  const float* real_src = MODE == X_QUOT ? p.phi : (MODE == X_UPDATE ? p.psi : p.acc);
+  const float* real_src = MODE == X_QUOT ? p.phi : (MODE == X_ACCUM ? p.acc : p.psi);
   const int ntiles = (int)((p.nrows + R - 1) / R);
   const int nrows_i = (int)p.nrows;
 
@@ -97,10 +99,12 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
     const int tile = p.reverse ? ntiles - 1 - t : t;
     const int row0 = tile * R;
     const int rv = min(R, nrows_i - row0);
-    if (tid == 0) mbar_expect_tx(&bars[1], (uint32_t)rv * (uint32_t)(p.nx * sizeof(float)));
+    if (tid == 0) mbar_expect_tx(&bars[1], (uint32_t)rv * (uint32_t)(p.nx * sizeof(float)) * (has_w ? 2u : 1u));
     __syncwarp();
-    for (int r = tid; r < rv; r += 32)
+    for (int r = tid; r < rv; r += 32) {
       bulk_g2s(rst + (size_t)r * RSTR, real_src + (long long)(row0 + r) * p.nx, p.nx * sizeof(float), &bars[1]);
+      if (has_w) bulk_g2s(wrst + (size_t)r * RSTR, p.wts + (long long)(row0 + r) * p.nx, p.nx * sizeof(float), &bars[1]);
+    }
   };
 
   const int rowA = tid / A, k1 = tid - rowA * A;
@@ -124,6 +128,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
       for (int i = tid; i < rv * p.nx; i += blockDim.x) {
         const int r = i / p.nx, x = i - r * p.nx;
         rst[(size_t)r * RSTR + x] = real_src[(long long)(row0 + r) * p.nx + x];
+        if (has_w) wrst[(size_t)r * RSTR + x] = p.wts[(long long)(row0 + r) * p.nx + x];
       }
     }
     mbar_wait(&bars[0], it & 1);
@@ -171,6 +176,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
     if (actB) {
       const long long rbase = (long long)growB * p.nx;
       const float* rrow = rst + (size_t)rowB * RSTR;
+      const float* wrow = wrst + (size_t)rowB * RSTR;
       float* prow = p.psi + rbase;
       float* arow = p.acc + rbase;
       const int lo_int = p.rx, hi_int = min(p.hx - p.rx, p.nx - p.hx);   // interior: no overlap, both halves live
@@ -179,8 +185,9 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
       auto voxel = [&](int x, float v) -> float {
         if constexpr (MODE == X_QUOT) {
           return __fdividef(rrow[x], fmaxf(v, p.eps));                    // S2, R4
-        } else if constexpr (MODE == X_UPDATE) {
+        } else if constexpr (MODE == X_UPDATE || MODE == X_UPDATE_W) {
           const float o = rrow[x];
+          if (has_w) v = fmaf(wrow[x], v - 1.f, 1.f);                     // section 12: fraction w of the RL step
           const float nw = fmaxf(o * v, p.psi_floor);                     // eq. 109-112, R4
           prow[x] = nw;
           flux += nw;
@@ -252,7 +259,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
   }
 
   // ---- per-CTA statistics of the update: {sum psi_new, sum |psi_new - psi_old|} ----------------
-  if (MODE == X_UPDATE || acc_last) {
+  if (MODE == X_UPDATE || MODE == X_UPDATE_W || acc_last) {
     double df = dflux, dl = dl1;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -515,9 +522,9 @@ struct LaunchTma {
   using Cfg = PassCfg<A, B>;
 
   // exchange rows are at most ROW_F2 + 16 float2 (the planner searches the conflict-free stride there)
-  static size_t xrow_smem(int rows, int rx, int nx) {
+  static size_t xrow_smem(int rows, int rx, int nx, int weighted) {
     return (size_t)rows * xrow_cstride(Cfg::M, A) * sizeof(float2) +
-           (size_t)rows * xrow_rstride(nx, B) * sizeof(float) + (size_t)rows * (Cfg::ROW_F2 + 16) * sizeof(float2) +
+           (size_t)(weighted ? 2 : 1) * rows * xrow_rstride(nx, B) * sizeof(float) + (size_t)rows * (Cfg::ROW_F2 + 16) * sizeof(float2) +
            (size_t)B * Cfg::AP * sizeof(float2) + (size_t)2 * rows * rx * sizeof(float) + 32;
   }
 
@@ -531,6 +538,7 @@ struct LaunchTma {
     MVD_SET((xrow_tma_kernel<A, B, X_QUOT>));
     MVD_SET((xrow_tma_kernel<A, B, X_UPDATE>));
     MVD_SET((xrow_tma_kernel<A, B, X_ACCUM>));
+    MVD_SET((xrow_tma_kernel<A, B, X_UPDATE_W>));
     MVD_SET((strided_tma_kernel<A, B, -1>));
     MVD_SET((strided_tma_kernel<A, B, 1>));
     MVD_SET((zconv_tma_kernel<A, B>));
@@ -544,7 +552,9 @@ struct LaunchTma {
         ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_QUOT>, nthreads, smem)
         : mode == X_UPDATE
         ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_UPDATE>, nthreads, smem)
-        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_ACCUM>, nthreads, smem);
+        : mode == X_ACCUM
+        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_ACCUM>, nthreads, smem)
+        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_UPDATE_W>, nthreads, smem);
     return e == cudaSuccess ? n : 0;
   }
 
@@ -581,10 +591,11 @@ struct LaunchTma {
 
   static cudaError_t xrow(const XArgs& a, int mode, cudaStream_t s) {
     if (a.grid <= 0) return cudaSuccess;
-    const size_t smem = xrow_smem(a.rows_per_cta, a.rx, a.nx);
+    const size_t smem = xrow_smem(a.rows_per_cta, a.rx, a.nx, mode == X_UPDATE_W);
     if (mode == X_QUOT) xrow_tma_kernel<A, B, X_QUOT><<<a.grid, a.nthreads, smem, s>>>(a);
     else if (mode == X_UPDATE) xrow_tma_kernel<A, B, X_UPDATE><<<a.grid, a.nthreads, smem, s>>>(a);
     else if (mode == X_ACCUM) xrow_tma_kernel<A, B, X_ACCUM><<<a.grid, a.nthreads, smem, s>>>(a);
+    else if (mode == X_UPDATE_W) xrow_tma_kernel<A, B, X_UPDATE_W><<<a.grid, a.nthreads, smem, s>>>(a);
     else return cudaErrorInvalidValue;
     return cudaGetLastError();
   }

@@ -388,3 +388,59 @@ def test_repeated_runs_are_bit_identical(mvd, config2):
     g, _ = gpu_checkpoints(mvd, config2, "efficient", "auto", (2,))
     h, _ = gpu_checkpoints(mvd, config2, "efficient", "auto", (2,))
     assert np.array_equal(g[2], h[2])
+
+
+# ------------------------------------------------------------------------------------------
+# section 12 (L891-903): per-view weights of partially overlapping views, sequential updates
+# ------------------------------------------------------------------------------------------
+def _partial_overlap_weights(shape, n_views):
+    """View v covers a box shifted along x (and y for odd v): cosine-blended, sum over views <= 1."""
+    nz, ny, nx = shape
+    ws = []
+    for v in range(n_views):
+        lo = (0, (ny // 6) * (v & 1), (nx // 8) * v)
+        hi = (nz, ny - (ny // 7) * ((v + 1) & 1), nx - (nx // 8) * (n_views - 1 - v))
+        ws.append(O.blending_weights(shape, lo, hi, border=5))
+    return O.normalise_weights(ws, 1.0)
+
+
+@pytest.mark.parametrize("dims,box", [((24, 20, 18), (5, 7, 9)), ((33, 17, 9), (3, 5, 7))])   # aligned rows / odd Nx
+def test_weighted_osem_matches_oracle(mvd, dims, box):
+    import torch
+    p = mvd_synth.make_tiny_asymmetric(dims=dims, psf_dims=box, n_views=3)
+    ws = _partial_overlap_weights(p.views[0].shape, 3)
+    wdev = [torch.from_numpy(w.astype(np.float32)).cuda() for w in ws]
+    w32 = [w.astype(np.float32).astype(np.float64) for w in ws]       # both sides see the same fp32 weights
+    for mode in ("auto", "plain"):
+        d = mvd.Deconvolver(to_dev(p.views), p.psfs, variant="osem", kernel_mode=mode, weights=wdev)
+        o = O.Oracle(p.views, p.psfs, "osem", kernel_mode=mode, weights=w32)
+        d.iterate(1)
+        o.iterate(1)
+        check(d.get_estimate_host(), o.psi, 1, "weighted %s" % mode)
+        d.iterate(4)
+        o.iterate(4)
+        check(d.get_estimate_host(), o.psi, 5, "weighted %s" % mode)
+        d.close()
+
+
+def test_weights_one_equal_no_weights_and_combined_variants_refuse(mvd, tiny):
+    import torch
+    ones = [torch.ones(tiny.views[0].shape, device="cuda") for _ in tiny.views]
+    a, _ = gpu_checkpoints(mvd, tiny, "osem", "auto", (3,))
+    b, _ = gpu_checkpoints(mvd, tiny, "osem", "auto", (3,), weights=ones)
+    l2, mx = errors(b[3], a[3])
+    assert l2 < 1e-6 and mx < 1e-5                                    # 1 + 1*(f-1) rounds once more than f
+    with pytest.raises(mvd.MvdError):
+        mvd.Deconvolver(to_dev(tiny.views), tiny.psfs, variant="efficient", weights=ones)
+
+
+def test_weighted_config2_size(mvd, config2):
+    """Weights at a size that spans many tiles: 128^3, 3 views, 5 iterations."""
+    import torch
+    ws = _partial_overlap_weights(config2.views[0].shape, 3)
+    wdev = [torch.from_numpy(w.astype(np.float32)).cuda() for w in ws]
+    w32 = [w.astype(np.float32).astype(np.float64) for w in ws]
+    g, _ = gpu_checkpoints(mvd, config2, "osem", "auto", (1, 5), weights=wdev, use_graph=True)
+    o, _ = oracle_checkpoints(config2, "osem", "auto", (1, 5), weights=w32)
+    check(g[1], o[1], 1, "weighted config 2")
+    check(g[5], o[5], 5, "weighted config 2")

@@ -290,3 +290,76 @@ def test_blocked_is_close_to_whole_in_block_interiors():
     rel = np.abs(whole - blk) / np.maximum(whole, 1e-6)
     assert np.median(rel) < 1e-2
     assert blk.shape == whole.shape and np.isfinite(blk).all()
+
+
+# --------------------------------------------------------------------------------------
+# section 12 (L891-903): weights of partially overlapping views
+# --------------------------------------------------------------------------------------
+def test_weights_interpolate_between_old_estimate_and_rl_step(tiny):
+    """L897: the weight is "the fraction of change suggested by a Lucy-Richardson update step":
+    per voxel psi_w = (1-w) psi + w psi_RL.  Checked against the (pinned) unweighted update, so a
+    wrong sign or a dropped '1 +' fails; w = 1 is the plain update, w = 0 leaves psi untouched."""
+    rng = np.random.default_rng(3)
+    views, psfs = tiny.views[:1], tiny.psfs[:1]
+    psi0 = rng.random(views[0].shape) * 50 + 1
+    plain = O.Oracle(views, psfs, "osem", kernel_mode="plain", psi0=psi0)
+    plain.iterate(1)
+    w = rng.random(views[0].shape)
+    w[:2] = 0.0
+    w[-2:] = 1.0
+    ow = O.Oracle(views, psfs, "osem", kernel_mode="plain", psi0=psi0, weights=[w])
+    ow.iterate(1)
+    assert np.allclose(ow.psi, (1 - w) * psi0 + w * plain.psi, rtol=1e-13, atol=0)
+    assert np.array_equal(ow.psi[:2], psi0[:2])
+    assert np.allclose(ow.psi[-2:], plain.psi[-2:], rtol=1e-14)
+
+
+def test_unit_weights_change_nothing_and_zero_view_is_skipped(tiny):
+    ones = [np.ones(tiny.views[0].shape)] * 3
+    a = O.deconvolve(tiny.views, tiny.psfs, "osem", 2)
+    b = O.deconvolve(tiny.views, tiny.psfs, "osem", 2, weights=ones)
+    assert np.allclose(a, b, rtol=1e-14)
+    # a view with weight 0 everywhere contributes nothing: same as running without that view's update
+    w = [np.ones(tiny.views[0].shape), np.zeros(tiny.views[0].shape), np.ones(tiny.views[0].shape)]
+    c = O.Oracle(tiny.views, tiny.psfs, "osem", kernel_mode="plain", weights=w)
+    c.iterate(1)
+    d = O.Oracle([tiny.views[0], tiny.views[2]], [tiny.psfs[0], tiny.psfs[2]], "osem", kernel_mode="plain",
+                 psi0=O.initial_estimate(tiny.views))
+    d.iterate(1)
+    assert np.allclose(c.psi, d.psi, rtol=1e-13)
+    with pytest.raises(ValueError):
+        O.Oracle(tiny.views, tiny.psfs, "efficient", weights=ones)
+
+
+def test_blending_weights_closed_form():
+    """L891: 1 in the central part, cosine ramp to 0 at the faces of the view's box, 0 outside."""
+    shape, lo, hi, border = (9, 30, 40), (0, 4, 10), (9, 26, 34), 6
+    w = O.blending_weights(shape, lo, hi, border)
+    assert w.min() >= 0 and w.max() <= 1
+    assert np.all(w[:, :4] == 0) and np.all(w[:, 26:] == 0) and np.all(w[:, :, :10] == 0) and np.all(w[:, :, 34:] == 0)
+    # along x through the centre of y (z spans 9 voxels with border 6: the z ramp is a constant factor)
+    line = w[4, 15, :]
+    zf, yf = 0.5 * (1 - np.cos(np.pi * 4.5 / 6)), 1.0
+    for x, d in ((10, 0.5), (12, 2.5), (13, 3.5), (33, 0.5), (31, 2.5)):
+        assert line[x] == pytest.approx(zf * yf * 0.5 * (1 - np.cos(np.pi * d / border)), rel=1e-12)
+    assert np.allclose(line[16:28], zf)                           # plateau
+    assert np.allclose(line[10:34], line[10:34][::-1])            # symmetric
+    assert np.all(np.diff(line[10:17]) > 0)                       # monotone ramp
+    # half-way up the ramp the weight is one half (cos(pi/2) = 0)
+    assert 0.5 * (1 - np.cos(np.pi * 3.0 / 6)) == pytest.approx(0.5)
+
+
+def test_normalise_weights_never_increases_and_caps_the_sum():
+    rng = np.random.default_rng(9)
+    ws = [rng.random((4, 5, 6)) for _ in range(4)]
+    for cap in (1.0, 2.0):
+        out = O.normalise_weights(ws, cap)
+        tot = np.sum(out, axis=0)
+        assert np.all(tot <= cap + 1e-12)
+        for a, b in zip(ws, out):
+            assert np.all(b <= a + 1e-15)                          # "never increased above 1" (L895)
+        untouched = np.sum(ws, axis=0) <= cap
+        for a, b in zip(ws, out):
+            assert np.array_equal(a[untouched], b[untouched])
+        capped = ~untouched
+        assert np.allclose(tot[capped], cap)
