@@ -337,10 +337,17 @@ def run_ours(args):
         del d, dev_views
         torch.cuda.empty_cache()
 
+        copy_stream = torch.cuda.Stream()
+
         def job():
-            with torch.cuda.stream(stream):
+            # the views are copied on their own stream; mvd_create waits for them (views_ready) only
+            # where it first reads them, so the copy overlaps the PSF precompute
+            with torch.cuda.stream(copy_stream):
                 dv = [h.to("cuda", non_blocking=True) for h in host_views]
-            dd = mvd.Deconvolver(dv, prob.psfs, variant="osem", stream=stream, use_graph=use_graph)
+                ready = torch.cuda.Event()
+                ready.record(copy_stream)
+            dd = mvd.Deconvolver(dv, prob.psfs, variant="osem", stream=stream, use_graph=use_graph,
+                                 views_ready=ready)
             dd.iterate(iters)
             dd.get_estimate_host(out_host.numpy())
             dd.close()

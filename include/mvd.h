@@ -94,6 +94,9 @@ typedef struct {
                                 * psi <- max(psi * (1 + w_v (f_v - 1)), floor).  MVD_OSEM only (else
                                 * MVD_ERR_UNSUPPORTED).  NULL -> no weights.  How the weights are built (cosine
                                 * blending, sum over views <= c) is the caller's business. */
+  void* views_ready;         /* optional cudaEvent_t: mvd_create makes its stream wait for it before the first read of
+                              * the views (the initial estimate), so the caller's host-to-device copy of the views
+                              * (on another stream) overlaps the PSF precompute.  NULL -> the views are ready. */
 } mvd_options;
 
 /* Fills *opt with the defaults (struct_size set, everything else 0/NULL/defaults). */

@@ -46,6 +46,7 @@ class mvd_options(C.Structure):
         ("stream", C.c_void_p),
         ("use_graph", C.c_int),
         ("weights", C.c_void_p),
+        ("views_ready", C.c_void_p),
     ]
 
 
@@ -170,7 +171,7 @@ class Deconvolver:
 
     def __init__(self, views, psfs, variant="osem", kernel_mode="auto", literal_product=False,
                  eps=None, psi_floor=None, psi0=None, fft_dims=None, use_graph=False, stream=None,
-                 weights=None):
+                 weights=None, views_ready=None):
         import torch
 
         lib = load_library()
@@ -215,6 +216,8 @@ class Deconvolver:
                 raise MvdError("weight images must have the shape of the views")
             self._weight_ptrs = (C.c_void_p * len(views))(*[w.data_ptr() for w in self._weights])
             opt.weights = C.cast(self._weight_ptrs, C.c_void_p)
+        if views_ready is not None:      # torch.cuda.Event recorded after the caller's copy of the views
+            opt.views_ready = views_ready.cuda_event
         self.workspace_bytes = int(nbytes)
         view_ptrs = (C.c_void_p * len(views))(*[v.data_ptr() for v in self.views])
         ctx = C.c_void_p()

@@ -906,6 +906,9 @@ mvd_status mvd_create(mvd_ctx** out, int n_views, const float* const* views, con
   }
 
   s = precompute(c, psfs);
+  if (s == MVD_OK && opt->views_ready &&
+      c->fail(cudaStreamWaitEvent(c->stream, reinterpret_cast<cudaEvent_t>(opt->views_ready), 0), "views_ready"))
+    s = MVD_ERR_CUDA;
   if (s == MVD_OK) s = init_estimate(c, opt->psi0);
   if (s == MVD_OK && c->fail(cudaStreamSynchronize(c->stream), "mvd_create")) s = MVD_ERR_CUDA;
   if (s != MVD_OK) {
@@ -1152,6 +1155,7 @@ extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* vi
   if (!views || !psfs || !dst || !opt_in || iterations < 0) return MVD_ERR_INVALID_ARG;
   mvd_options tmp;
   const mvd_options* opt = defaults(opt_in, &tmp);
+  if (opt->weights || opt->views_ready) return MVD_ERR_UNSUPPORTED;   // whole-volume options
   BlockedLayout L;
   mvd_status s = blocked_layout(L, n_views, dims, psf_dims, variant, opt, block_dims, halo);
   if (s != MVD_OK) return s;
