@@ -94,6 +94,12 @@ typedef struct {
                                 * psi <- max(psi * (1 + w_v (f_v - 1)), floor).  MVD_OSEM only (else
                                 * MVD_ERR_UNSUPPORTED).  NULL -> no weights.  How the weights are built (cosine
                                 * blending, sum over views <= c) is the caller's business. */
+  const int* local_views;    /* view-parallel combined variants: indices (ascending, unique) of the views THIS context owns;
+                              * NULL -> all.  All n_views PSFs are still given (the compound kernels need them), views[v]
+                              * may be NULL for views not listed.  Such a context is driven by mvd_partial_product /
+                              * mvd_apply_product, not mvd_iterate; psi0 or psi0_value must be given. */
+  int n_local;               /* length of local_views */
+  float psi0_value;          /* > 0: constant initial estimate (a multi-rank caller passes the mean over ALL views) */
   void* views_ready;         /* optional cudaEvent_t: mvd_create makes its stream wait for it before the first read of
                               * the views (the initial estimate), so the caller's host-to-device copy of the views
                               * (on another stream) overlaps the PSF precompute.  NULL -> the views are ready. */
@@ -110,6 +116,24 @@ MVD_API size_t mvd_workspace_size(int n_views, const int dims[3], const int (*ps
 /* The FFT lengths {Mx2, My, Mz} the library would use (for reporting algorithmic bytes). */
 MVD_API mvd_status mvd_plan_dims(int n_views, const int dims[3], const int (*psf_dims)[3],
                          const mvd_options* opt, int fft_dims_out[3]);
+
+/* View-parallel form of the combined variants ("all view contributions can be computed at the same
+ * time"; eq. 70 / 104 with the root of eq. 44).  Each rank owns some views and the same psi:
+ *   mvd_partial_product : acc <- prod over the context's own views of max(f_v, 0) (f_v itself if literal_product),
+ *                         every f_v computed from the current psi; psi is not changed.  Asynchronous.
+ *   mvd_get_product     : DEVICE pointer to acc (N voxels, fp32, inside the workspace): the caller multiplies the
+ *                         ranks' partial products element-wise in place (one all-reduce with the PRODUCT operator).
+ *   mvd_apply_product   : psi <- max(psi * acc^(1/total_views), floor) (no root if literal_product), statistics;
+ *                         counts as one iteration.  Every rank applies the same product, so psi stays replicated.
+ * MVD_INDEPENDENT / MVD_EFFICIENT only (MVD_ERR_UNSUPPORTED for MVD_OSEM: sequential updates do not split).
+ * mvd_reduce_sum: sum of n device floats in fp64 -> *host_out (for the global mean of the views); scratch = DEVICE
+ * memory of at least mvd_reduce_scratch_bytes(). */
+MVD_API mvd_status mvd_partial_product(mvd_ctx* ctx);
+MVD_API mvd_status mvd_get_product(mvd_ctx* ctx, float** acc_device);
+MVD_API mvd_status mvd_apply_product(mvd_ctx* ctx, int total_views);
+MVD_API size_t mvd_reduce_scratch_bytes(void);
+MVD_API mvd_status mvd_reduce_sum(const float* src_device, long long n, void* scratch_device, void* stream,
+                                  double* host_out);
 
 /* Builds a context: normalises the PSFs, computes the back-projectors K_v on the device (eq. 105 /
  * 107 / 108), their spectra and those of P_v, and the initial estimate.  Synchronises the stream

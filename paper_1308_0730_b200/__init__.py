@@ -11,6 +11,9 @@ from .binding import (  # noqa: F401
     VARIANTS,
     Deconvolver,
     MvdError,
+    ViewParallelDeconvolver,
+    reduce_sum,
+    split_views,
     deconvolve_blocked,
     load_library,
     plan_dims,

@@ -25,6 +25,7 @@ SYMBOLS = (
     "mvd_get_estimate", "mvd_set_estimate", "mvd_get_stats", "mvd_get_back_projector", "mvd_convolve",
     "mvd_launch_count", "mvd_profile", "mvd_profile_read", "mvd_kernel_class_name", "mvd_blocked_workspace_size", "mvd_deconvolve_blocked", "mvd_destroy",
     "mvd_status_string", "mvd_last_error",
+    "mvd_partial_product", "mvd_get_product", "mvd_apply_product", "mvd_reduce_scratch_bytes", "mvd_reduce_sum",
 )
 
 
@@ -46,6 +47,9 @@ class mvd_options(C.Structure):
         ("stream", C.c_void_p),
         ("use_graph", C.c_int),
         ("weights", C.c_void_p),
+        ("local_views", C.c_void_p),
+        ("n_local", C.c_int),
+        ("psi0_value", C.c_float),
         ("views_ready", C.c_void_p),
     ]
 
@@ -105,6 +109,16 @@ def load_library():
     lib.mvd_status_string.restype = C.c_char_p
     lib.mvd_last_error.argtypes = [vp]
     lib.mvd_last_error.restype = C.c_char_p
+    lib.mvd_partial_product.argtypes = [vp]
+    lib.mvd_partial_product.restype = C.c_int
+    lib.mvd_get_product.argtypes = [vp, C.POINTER(vp)]
+    lib.mvd_get_product.restype = C.c_int
+    lib.mvd_apply_product.argtypes = [vp, C.c_int]
+    lib.mvd_apply_product.restype = C.c_int
+    lib.mvd_reduce_scratch_bytes.argtypes = []
+    lib.mvd_reduce_scratch_bytes.restype = C.c_size_t
+    lib.mvd_reduce_sum.argtypes = [vp, C.c_longlong, vp, vp, C.POINTER(C.c_double)]
+    lib.mvd_reduce_sum.restype = C.c_int
     _lib = lib
     return lib
 
@@ -171,28 +185,46 @@ class Deconvolver:
 
     def __init__(self, views, psfs, variant="osem", kernel_mode="auto", literal_product=False,
                  eps=None, psi_floor=None, psi0=None, fft_dims=None, use_graph=False, stream=None,
-                 weights=None, views_ready=None):
+                 weights=None, views_ready=None, local_views=None, psi0_value=None):
         import torch
 
         lib = load_library()
         if not torch.cuda.is_available():
             raise MvdError("no CUDA device: the multi-view deconvolution path has no CPU fallback")
-        if len(views) != len(psfs) or not views:
+        if local_views is not None:
+            # view-parallel context: `views` holds this rank's views only, in the order of local_views
+            local_views = [int(v) for v in local_views]
+            if len(views) != len(local_views):
+                raise MvdError("need one view per entry of local_views")
+            full = [None] * len(psfs)
+            for i, v in enumerate(local_views):
+                full[v] = views[i]
+            self._local = (C.c_int * len(local_views))(*local_views)
+        else:
+            full = list(views)
+        if len(full) != len(psfs) or not views:
             raise MvdError("need one PSF per view")
         self._torch = torch
-        self.views = [v if (v.is_cuda and v.dtype == torch.float32 and v.is_contiguous())
-                      else v.to(device="cuda", dtype=torch.float32).contiguous() for v in views]
-        shape = tuple(self.views[0].shape)
-        if len(shape) != 3 or any(tuple(v.shape) != shape for v in self.views):
+        self.views = [None if v is None else
+                      (v if (v.is_cuda and v.dtype == torch.float32 and v.is_contiguous())
+                       else v.to(device="cuda", dtype=torch.float32).contiguous()) for v in full]
+        present = [v for v in self.views if v is not None]
+        shape = tuple(present[0].shape)
+        if len(shape) != 3 or any(tuple(v.shape) != shape for v in present):
             raise MvdError("views must be 3-D tensors of one shape (Nz, Ny, Nx)")
         self.shape = shape
         self.dims = (shape[2], shape[1], shape[0])
-        self.device = self.views[0].device
+        self.device = present[0].device
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._psfs, psf_ptrs, psf_dims = _psf_args(psfs)
         self._psf_dims = psf_dims
         opt = _make_options(kernel_mode, literal_product, eps, psi_floor, fft_dims, use_graph)
-        nbytes = lib.mvd_workspace_size(len(views), _Int3(*self.dims), C.cast(psf_dims, C.c_void_p),
+        if local_views is not None:
+            opt.local_views = C.cast(self._local, C.c_void_p)
+            opt.n_local = len(local_views)
+        if psi0_value is not None:
+            opt.psi0_value = float(psi0_value)
+        nbytes = lib.mvd_workspace_size(len(full), _Int3(*self.dims), C.cast(psf_dims, C.c_void_p),
                                         VARIANTS[variant], C.byref(opt))
         if nbytes == 0:
             raise MvdError("mvd_workspace_size: invalid or unsupported problem "
@@ -209,32 +241,49 @@ class Deconvolver:
             opt.psi0 = self._psi0.data_ptr()
         self._weights = None
         if weights is not None:
-            if len(weights) != len(views):
+            if len(weights) != len(full):
                 raise MvdError("need one weight image per view")
             self._weights = [w.to(device=self.device, dtype=torch.float32).contiguous() for w in weights]
             if any(tuple(w.shape) != shape for w in self._weights):
                 raise MvdError("weight images must have the shape of the views")
-            self._weight_ptrs = (C.c_void_p * len(views))(*[w.data_ptr() for w in self._weights])
+            self._weight_ptrs = (C.c_void_p * len(full))(*[w.data_ptr() for w in self._weights])
             opt.weights = C.cast(self._weight_ptrs, C.c_void_p)
         if views_ready is not None:      # torch.cuda.Event recorded after the caller's copy of the views
             opt.views_ready = views_ready.cuda_event
         self.workspace_bytes = int(nbytes)
-        view_ptrs = (C.c_void_p * len(views))(*[v.data_ptr() for v in self.views])
+        view_ptrs = (C.c_void_p * len(full))(*[None if v is None else v.data_ptr() for v in self.views])
         ctx = C.c_void_p()
         with torch.cuda.device(self.device):
-            st = lib.mvd_create(C.byref(ctx), len(views), view_ptrs, _Int3(*self.dims), psf_ptrs,
+            st = lib.mvd_create(C.byref(ctx), len(full), view_ptrs, _Int3(*self.dims), psf_ptrs,
                                 C.cast(psf_dims, C.c_void_p), VARIANTS[variant], C.byref(opt))
         _check(st, None, "mvd_create")
         self._ctx = ctx
         self._lib = lib
         out = _Int3()
-        lib.mvd_plan_dims(len(views), _Int3(*self.dims), C.cast(psf_dims, C.c_void_p), C.byref(opt), out)
+        lib.mvd_plan_dims(len(full), _Int3(*self.dims), C.cast(psf_dims, C.c_void_p), C.byref(opt), out)
         self.fft_dims = tuple(out)
 
     # -- C ABI mirrors --------------------------------------------------------------------------
     def iterate(self, n=1):
         with self._torch.cuda.device(self.device):
             _check(self._lib.mvd_iterate(self._ctx, int(n)), self._ctx, "mvd_iterate")
+
+    def partial_product(self):
+        """mvd_partial_product: acc <- product over this context's views of max(f_v, 0), psi unchanged."""
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.mvd_partial_product(self._ctx), self._ctx, "mvd_partial_product")
+
+    def product_tensor(self):
+        """The product accumulator as a float32 tensor (Nz,Ny,Nx) aliasing the workspace (mvd_get_product)."""
+        p = C.c_void_p()
+        _check(self._lib.mvd_get_product(self._ctx, C.byref(p)), self._ctx, "mvd_get_product")
+        off = p.value - self.workspace.data_ptr()
+        n = self.shape[0] * self.shape[1] * self.shape[2]
+        return self.workspace[off:off + 4 * n].view(self._torch.float32).view(self.shape)
+
+    def apply_product(self, total_views):
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.mvd_apply_product(self._ctx, int(total_views)), self._ctx, "mvd_apply_product")
 
     def get_estimate(self, out=None):
         """Device tensor (Nz,Ny,Nx) with a copy of psi (asynchronous on the stream)."""
@@ -346,3 +395,77 @@ def deconvolve_blocked(views, psfs, block_dims, iterations, variant="osem", kern
     stream.synchronize()
     del keep
     return dst, int(launches.value)
+
+
+def reduce_sum(t, stream=None):
+    """mvd_reduce_sum: fp64 sum of a CUDA float32 tensor through the library's reduction kernels."""
+    import torch
+    lib = load_library()
+    t = t.contiguous()
+    stream = stream if stream is not None else torch.cuda.current_stream(t.device)
+    with torch.cuda.stream(stream):
+        scratch = torch.empty(int(lib.mvd_reduce_scratch_bytes()), dtype=torch.uint8, device=t.device)
+    out = C.c_double(0.0)
+    with torch.cuda.device(t.device):
+        _check(lib.mvd_reduce_sum(t.data_ptr(), t.numel(), scratch.data_ptr(), stream.cuda_stream, C.byref(out)),
+               None, "mvd_reduce_sum")
+    return float(out.value)
+
+
+def split_views(n_views, world, rank):
+    """Views of `rank` when n_views are dealt round-robin over `world` ranks (ascending indices)."""
+    return [v for v in range(n_views) if v % world == rank]
+
+
+class ViewParallelDeconvolver:
+    """Combined variants (independent / efficient) with the views split over the ranks of a
+    torch.distributed process group (all view contributions can be computed at the
+    same time).  Every rank keeps the whole estimate; one iteration = each rank's partial product
+    of its views' factors, ONE all-reduce(PRODUCT) of N floats, the same root update on every rank.
+    `local_views_data`: this rank's views (CUDA tensors) in the order of split_views(); `psfs`:
+    ALL PSFs (the compound kernels need them).  group=None and world 1 runs without torch.distributed."""
+
+    def __init__(self, local_views_data, psfs, variant="efficient", rank=0, world=1, group=None, **kw):
+        import torch
+        if variant not in ("independent", "efficient"):
+            raise MvdError("sequential updates (osem) do not split over ranks")
+        self.rank, self.world, self.group = int(rank), int(world), group
+        self.n_views = len(psfs)
+        self.local = split_views(self.n_views, self.world, self.rank)
+        if not self.local or len(local_views_data) != len(self.local):
+            raise MvdError("rank %d owns views %s" % (self.rank, self.local))
+        self._torch = torch
+        stream = kw.pop("stream", None) or torch.cuda.current_stream(local_views_data[0].device)
+        # psi^0 = mean over ALL views (L304, L421): local sums by the library, one all-reduce(SUM)
+        tot = torch.tensor([sum(reduce_sum(v, stream) for v in local_views_data),
+                            float(sum(v.numel() for v in local_views_data))], dtype=torch.float64)
+        tot = self._all_reduce(tot, "sum")
+        self.d = Deconvolver(local_views_data, psfs, variant=variant, local_views=self.local,
+                             psi0_value=float(tot[0] / tot[1]), stream=stream, **kw)
+
+    def _all_reduce(self, t, op):
+        if self.world == 1:
+            return t
+        import torch.distributed as dist
+        if t.device.type == "cpu" and dist.get_backend(self.group) == "nccl":
+            t = t.cuda()
+        dist.all_reduce(t, op=dist.ReduceOp.SUM if op == "sum" else dist.ReduceOp.PRODUCT, group=self.group)
+        return t.cpu() if op == "sum" else t
+
+    def iterate(self, n=1):
+        torch = self._torch
+        for _ in range(int(n)):
+            self.d.partial_product()
+            if self.world > 1:
+                with torch.cuda.stream(self.d.stream):      # the collective is ordered after the kernels
+                    self._all_reduce(self.d.product_tensor(), "product")
+            self.d.apply_product(self.n_views)
+
+    def get_estimate_host(self, out=None):
+        return self.d.get_estimate_host(out)
+
+    def get_stats(self):
+        return self.d.get_stats()
+
+    def close(self):
+        self.d.close()

@@ -199,6 +199,36 @@ __global__ void paste_block_kernel(const float* __restrict__ src, Dims3 E, Dims3
   }
 }
 
+__global__ void fill_value_kernel(float* __restrict__ a, long long n, float value) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) a[i] = value;
+}
+
+// view-parallel combined update (eq. 70 / 104 with the root of eq. 44): acc holds the product of
+// max(f_v, 0) over ALL views; psi <- max(psi * acc^(1/V), floor); per-block {sum psi, sum |dpsi|}
+__global__ void __launch_bounds__(256) apply_product_kernel(float* __restrict__ psi, const float* __restrict__ acc,
+                                                            long long n, float inv_nviews, int literal,
+                                                            float psi_floor, double* __restrict__ partials) {
+  __shared__ double red[32];
+  double flux = 0.0, l1 = 0.0;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    float f = acc[i];
+    if (!literal && inv_nviews != 1.f) f = powf(f, inv_nviews);
+    const float o = psi[i];
+    const float nw = fmaxf(o * f, psi_floor);
+    psi[i] = nw;
+    flux += nw;
+    l1 += fabsf(nw - o);
+  }
+  flux = block_sum(flux, red);
+  l1 = block_sum(l1, red);
+  if (threadIdx.x == 0) {
+    partials[2 * (size_t)blockIdx.x] = flux;
+    partials[2 * (size_t)blockIdx.x + 1] = l1;
+  }
+}
+
 __global__ void fill_const_kernel(float* __restrict__ a, long long n, const float* __restrict__ value) {
   const float m = *value;
   const long long stride = (long long)gridDim.x * blockDim.x;

@@ -345,6 +345,9 @@ struct mvd_ctx {
   char* ws = nullptr;
   std::vector<const float*> views;
   std::vector<const float*> weights;   // empty or one per view (borrowed)
+  std::vector<char> is_local;          // view-parallel contexts: which views this context owns (all by default)
+  bool partial = false;
+  float psi0_value = 0.f;
   bool w_valid = false;        // the work buffer holds the x-forward transform of the current psi
   bool broken = false;
   bool stats_valid = false;
@@ -750,6 +753,7 @@ mvd_status precompute(mvd_ctx* c, const float* const* psfs_host) {
     }
   }
   for (int v = 0; v < P.V; ++v) {
+    if (!c->is_local[v]) continue;
     const Dims3 K = P.K[v];
     const long long tot = (long long)K.x * K.y * K.z;
     const unsigned g256 = (unsigned)((tot + 255) / 256), g128 = (unsigned)((tot + 31) / 32);   // corr: one block of 256 threads per 32 taps
@@ -777,6 +781,7 @@ mvd_status precompute(mvd_ctx* c, const float* const* psfs_host) {
   }
   // spectra of P_v and K_v
   for (int v = 0; v < P.V; ++v) {
+    if (!c->is_local[v]) continue;
     MVD_TRY(build_spectrum(c, c->psf(v), P.K[v], c->specH(v)));
     MVD_TRY(build_spectrum(c, c->kern(v), P.K[v], c->specK(v)));
   }
@@ -787,6 +792,13 @@ mvd_status init_estimate(mvd_ctx* c, const float* psi0) {
   const Plan& P = c->P;
   if (psi0) {
     MVD_CK(cudaMemcpyAsync(c->psi(), psi0, sizeof(float) * P.nvox, cudaMemcpyDeviceToDevice, c->stream), "psi0 copy");
+  } else if (c->psi0_value > 0.f) {
+    fill_value_kernel<<<1184, 256, 0, c->stream>>>(c->psi(), P.nvox, c->psi0_value);
+    MVD_CK(cudaGetLastError(), "fill_value_kernel");
+    ++c->launches;
+  } else if (c->partial) {
+    snprintf(c->err, sizeof(c->err), "a view-parallel context needs psi0 or psi0_value");
+    return MVD_ERR_INVALID_ARG;
   } else {
     // psi^0 = average intensity over all views (L304, L421)
     for (int v = 0; v < P.V; ++v) {
@@ -857,10 +869,24 @@ mvd_status mvd_create(mvd_ctx** out, int n_views, const float* const* views, con
   if (!views || !psfs || !dims || !psf_dims || !opt_in) return MVD_ERR_INVALID_ARG;
   mvd_options tmp;
   const mvd_options* opt = defaults(opt_in, &tmp);
+  if (n_views < 1) return MVD_ERR_INVALID_ARG;
+  std::vector<char> is_local((size_t)n_views, opt->local_views ? 0 : 1);
+  if (opt->local_views) {
+    if (variant == MVD_OSEM) return MVD_ERR_UNSUPPORTED;      // sequential updates do not split over ranks
+    if (opt->n_local < 1 || opt->weights) return MVD_ERR_INVALID_ARG;
+    for (int i = 0; i < opt->n_local; ++i) {
+      const int v = opt->local_views[i];
+      if (v < 0 || v >= n_views || is_local[v] || (i > 0 && v <= opt->local_views[i - 1])) return MVD_ERR_INVALID_ARG;
+      is_local[v] = 1;
+    }
+  }
   for (int v = 0; v < n_views; ++v)
-    if (!views[v] || !psfs[v]) return MVD_ERR_INVALID_ARG;
+    if ((is_local[v] && !views[v]) || !psfs[v]) return MVD_ERR_INVALID_ARG;
   mvd_ctx* c = new (std::nothrow) mvd_ctx();
   if (!c) return MVD_ERR_INVALID_ARG;
+  c->is_local = is_local;
+  c->partial = opt->local_views != nullptr;
+  c->psi0_value = opt->psi0_value;
   mvd_status s = make_plan(c->P, n_views, dims, psf_dims, variant, opt);
   if (s != MVD_OK) { delete c; return s; }
   if (!opt->workspace || (reinterpret_cast<size_t>(opt->workspace) & 255) || opt->workspace_bytes < c->P.total) {
@@ -922,7 +948,7 @@ mvd_status mvd_create(mvd_ctx** out, int n_views, const float* const* views, con
 
 mvd_status mvd_iterate(mvd_ctx* c, int n) {
   if (!c || n < 0) return MVD_ERR_INVALID_ARG;
-  if (c->broken) return MVD_ERR_STATE;
+  if (c->broken || c->partial) return MVD_ERR_STATE;   // view-parallel contexts: mvd_partial_product / mvd_apply_product
   if (n == 0) return MVD_OK;
   MVD_TRY(ensure_w(c));
   if (c->use_graph) {
@@ -950,6 +976,69 @@ mvd_status mvd_iterate(mvd_ctx* c, int n) {
     MVD_TRY(iteration_body(c));
     ++c->iters;
   }
+  return MVD_OK;
+}
+
+mvd_status mvd_partial_product(mvd_ctx* c) {
+  if (!c) return MVD_ERR_INVALID_ARG;
+  if (c->broken) return MVD_ERR_STATE;
+  const Plan& P = c->P;
+  if (!P.combined) return MVD_ERR_UNSUPPORTED;
+  MVD_TRY(ensure_w(c));
+  // eq. 70 / 104: every f_v of this context's views from the same psi; the x and y forward passes of psi are shared
+  MVD_TRY(y_pass(c, c->W0(), -1, P.N[2], false));
+  bool first = true;
+  for (int v = 0; v < P.V; ++v) {
+    if (!c->is_local[v]) continue;
+    const int rx = (P.K[v].x - 1) / 2;
+    MVD_TRY(conv_core(c, c->W0(), c->W(), c->specH(v), true));
+    XArgs q = x_args(c, c->W(), c->W(), rx);
+    q.phi = c->views[v];
+    MVD_TRY(x_pass(c, q, X_QUOT));
+    MVD_TRY(conv_core(c, nullptr, c->W(), c->specK(v), false));
+    XArgs u = x_args(c, c->W(), c->W0(), rx);
+    u.acc_mode = first ? ACC_FIRST : ACC_MID;
+    first = false;
+    MVD_TRY(x_pass(c, u, X_ACCUM));
+  }
+  c->w_valid = false;            // the y pass ran in place on W0: it no longer holds the x transform of psi
+  return MVD_OK;
+}
+
+mvd_status mvd_get_product(mvd_ctx* c, float** acc_device) {
+  if (!c || !acc_device) return MVD_ERR_INVALID_ARG;
+  *acc_device = c->acc();
+  return MVD_OK;
+}
+
+mvd_status mvd_apply_product(mvd_ctx* c, int total_views) {
+  if (!c || total_views < 1) return MVD_ERR_INVALID_ARG;
+  if (c->broken) return MVD_ERR_STATE;
+  const Plan& P = c->P;
+  if (!P.combined) return MVD_ERR_UNSUPPORTED;
+  apply_product_kernel<<<P.sum_blocks, 256, 0, c->stream>>>(c->psi(), c->acc(), P.nvox, 1.0f / (float)total_views,
+                                                          c->literal, c->psi_floor, c->partials());
+  MVD_CK(cudaGetLastError(), "apply_product_kernel");
+  ++c->launches;
+  c->w_valid = false;
+  c->stats_valid = true;
+  c->stats_ncta = P.sum_blocks;
+  ++c->iters;
+  return MVD_OK;
+}
+
+size_t mvd_reduce_scratch_bytes(void) { return sizeof(double) * (1184 + 8); }
+
+mvd_status mvd_reduce_sum(const float* src, long long n, void* scratch, void* stream, double* host_out) {
+  if (!src || n < 0 || !scratch || !host_out) return MVD_ERR_INVALID_ARG;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  double* part = reinterpret_cast<double*>(scratch);
+  sum_f32_kernel<<<1184, 256, 0, st>>>(src, n, part);
+  final_sum_kernel<<<1, 256, 0, st>>>(part, 1184, 1, part + 1184);
+  if (cudaGetLastError() != cudaSuccess) return MVD_ERR_CUDA;
+  if (cudaMemcpyAsync(host_out, part + 1184, sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+      cudaStreamSynchronize(st) != cudaSuccess)
+    return MVD_ERR_CUDA;
   return MVD_OK;
 }
 

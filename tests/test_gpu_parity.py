@@ -444,3 +444,51 @@ def test_weighted_config2_size(mvd, config2):
     o, _ = oracle_checkpoints(config2, "osem", "auto", (1, 5), weights=w32)
     check(g[1], o[1], 1, "weighted config 2")
     check(g[5], o[5], 5, "weighted config 2")
+
+
+# ------------------------------------------------------------------------------------------
+# view-parallel combined variants (L815): two "ranks" emulated on one GPU as two
+# contexts that own different views; their partial products are multiplied as the all-reduce would
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", ["independent", "efficient"])
+def test_view_parallel_two_emulated_ranks(mvd, tiny, variant):
+    import torch
+    V = len(tiny.views)
+    views = to_dev(tiny.views)
+    mean = sum(mvd.reduce_sum(v) for v in views) / sum(v.numel() for v in views)
+    assert mean == pytest.approx(float(np.mean([v.astype(np.float64).mean() for v in tiny.views])), rel=1e-12)
+    ranks = []
+    for r in range(2):
+        loc = mvd.split_views(V, 2, r)
+        ranks.append(mvd.Deconvolver([views[v] for v in loc], tiny.psfs, variant=variant, local_views=loc,
+                                     psi0_value=mean))
+    o = O.Oracle(tiny.views, tiny.psfs, variant)
+    for it in range(3):
+        for d in ranks:
+            d.partial_product()
+        torch.cuda.synchronize()
+        prod = ranks[0].product_tensor() * ranks[1].product_tensor()      # = all-reduce(PRODUCT)
+        for d in ranks:
+            d.product_tensor().copy_(prod)
+            d.apply_product(V)
+        o.iterate(1)
+        a, b = ranks[0].get_estimate_host(), ranks[1].get_estimate_host()
+        assert np.array_equal(a, b)                                          # psi stays replicated
+        check(a, o.psi, it + 1, "view-parallel %s" % variant)
+    st = ranks[0].get_stats()
+    assert st["flux"] == pytest.approx(o.flux, rel=1e-5) and st["iterations_done"] == 3
+    with pytest.raises(mvd.MvdError):
+        ranks[0].iterate(1)                                                  # split contexts do not iterate alone
+    for d in ranks:
+        d.close()
+    with pytest.raises(mvd.MvdError):
+        mvd.Deconvolver([views[0]], tiny.psfs, variant="osem", local_views=[0], psi0_value=mean)
+
+
+def test_view_parallel_driver_world_1_equals_oracle(mvd, tiny):
+    d = mvd.ViewParallelDeconvolver(to_dev(tiny.views), tiny.psfs, variant="efficient")
+    d.iterate(2)
+    o = O.Oracle(tiny.views, tiny.psfs, "efficient")
+    o.iterate(2)
+    check(d.get_estimate_host(), o.psi, 2, "view-parallel driver")
+    d.close()
