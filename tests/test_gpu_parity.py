@@ -492,3 +492,56 @@ def test_view_parallel_driver_world_1_equals_oracle(mvd, tiny):
     o.iterate(2)
     check(d.get_estimate_host(), o.psi, 2, "view-parallel driver")
     d.close()
+
+
+# ------------------------------------------------------------------------------------------
+# every compiled pencil length (csrc/lengths.def), on every axis: one 'same' convolution with the
+# FFT length of that axis forced, against the oracle.  Covers every register transform (radices
+# 2,3,4,5,7 in all their mixes), the TMA-staged y/z passes and the x pass for every (A, B).
+# ------------------------------------------------------------------------------------------
+def _compiled_lengths():
+    import os
+    import re
+    path = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "paper_1308_0730_b200", "csrc",
+                        "lengths.def")
+    out = []
+    for line in open(path):
+        m = re.match(r"\s*MVD_LEN\((\d+),\s*(\d+)\)", line)
+        if m:
+            out.append(int(m.group(1)) * int(m.group(2)))
+    return sorted(out)
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_every_compiled_length_on_every_axis(mvd, axis):
+    import torch
+    rng = np.random.default_rng([7, axis])
+    box = (5, 5, 5)                                   # (Kx,Ky,Kz), r = 2
+    psf = mvd_synth.generate.random_psf(rng, box)
+    pn = O.normalise(psf)
+    tested = 0
+    for M in _compiled_lengths():
+        if M < 8 or (axis == 0 and M % 2):            # x lengths are even (16-byte rows)
+            continue
+        dims = [6, 7, 5]
+        dims[axis] = 2 * (M - 4) if axis == 0 else M - 2          # the largest volume this length serves
+        if dims[axis] < 3:
+            continue
+        fft = [0, 0, 0]
+        fft[axis] = M
+        view = (rng.random((dims[2], dims[1], dims[0]), dtype=np.float32) * 10 + 1)
+        d = mvd.Deconvolver([torch.from_numpy(view).cuda()], [psf], variant="osem", kernel_mode="plain",
+                            fft_dims=tuple(fft))
+        assert d.fft_dims[axis] == M
+        for which, k in ((0, pn), (1, O.flip(pn))):
+            got = d.convolve(0, which, torch.from_numpy(view).cuda()).cpu().numpy()
+            l2, mx = errors(got, O.same_fft(view, k))
+            assert l2 < 3e-6 and mx < 1e-4, (axis, M, which, l2, mx)
+        # and the fused x kernels (quotient, update) of this length: one OSEM iteration against the oracle
+        d.iterate(1)
+        o = O.Oracle([view], [psf], "osem", kernel_mode="plain")
+        o.iterate(1)
+        check(d.get_estimate_host(), o.psi, 1, "length %d axis %d" % (M, axis))
+        d.close()
+        tested += 1
+    assert tested >= 50
