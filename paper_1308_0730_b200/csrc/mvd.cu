@@ -272,8 +272,8 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
     }
     P.ytma = env_int("MVD_YTMA", 1);
     P.ztma = env_int("MVD_ZTMA", 1);
-    if (!plan_tma(P.ly, P.Mx, env_int("MVD_TYT", 0), (size_t)env_int("MVD_YT_SMEM_KB", 72) * 1024, false, &P.Tyt, &P.ntyt, &P.ybox, &P.ynbox)) P.ytma = 0;
-    if (!plan_tma(P.lz, P.Mx, env_int("MVD_TZT", 0), (size_t)env_int("MVD_ZT_SMEM_KB", 110) * 1024, true, &P.Tzt, &P.ntzt, &P.zbox, &P.znbox)) P.ztma = 0;
+    if (!plan_tma(P.ly, P.Mx, 0, (size_t)env_int("MVD_YT_SMEM_KB", 72) * 1024, false, &P.Tyt, &P.ntyt, &P.ybox, &P.ynbox)) P.ytma = 0;
+    if (!plan_tma(P.lz, P.Mx, 0, (size_t)env_int("MVD_ZT_SMEM_KB", 110) * 1024, true, &P.Tzt, &P.ntzt, &P.zbox, &P.znbox)) P.ztma = 0;
   }
   {
     // TMA-staged x pass (quotient / OSEM update): rows per tile sized for >= 3 resident CTAs per SM
@@ -476,7 +476,6 @@ mvd_status y_pass_tma(mvd_ctx* c, float2* buf, int dir, int nz_planes, int xt0, 
   a.reverse = c->use_flip ? (c->flip ^= 1) : 0;
   int& bl = c->yt_blocks[dir < 0 ? 0 : 1];
   if (bl == 0) bl = P.ly->strided_tma_blocks_per_sm(dir, a.nthreads, P.ly->strided_tma_smem(a.T, a.boxr, a.nbox, a.nst));
-  if (env_int("MVD_YBLK", 0) > 0) bl = std::min(bl, env_int("MVD_YBLK", 0));
   if (bl <= 0) { snprintf(c->err, sizeof(c->err), "y pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
   a.grid = (int)std::min<long long>((long long)n_xt * nz_planes, (long long)c->num_sms * bl);
   {
@@ -501,7 +500,6 @@ mvd_status z_conv_tma(mvd_ctx* c, const float2* in, float2* out, const float2* s
   a.xt0 = xt0; a.n_xt = n_xt;
   a.mx = P.Mx; a.my = P.My; a.plane = P.plane; a.nz = P.N[2]; a.nst_in = P.znst;
   if (c->zt_blocks == 0) c->zt_blocks = P.lz->zconv_tma_blocks_per_sm(a.nthreads, P.lz->zconv_tma_smem(a.T, a.boxr, a.nbox, a.nst_in));
-  if (env_int("MVD_ZBLK", 0) > 0) c->zt_blocks = std::min(c->zt_blocks, env_int("MVD_ZBLK", 0));
   if (c->zt_blocks <= 0) { snprintf(c->err, sizeof(c->err), "z pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
   a.grid = (int)std::min<long long>((long long)n_xt * ((P.My + 1) / 2), (long long)c->num_sms * c->zt_blocks);
   {
@@ -598,7 +596,6 @@ mvd_status x_pass(mvd_ctx* c, const XArgs& a_in, int mode) {
                   ((reinterpret_cast<size_t>(a.wts) & 15) == 0);
     if (c->xt_blocks[mode] == 0) {
       c->xt_blocks[mode] = P.lx->xrow_tma_blocks_per_sm(mode, a.nthreads, P.lx->xrow_tma_smem(a.rows_per_cta, P.r[0], P.N[0], mode == X_UPDATE_W));
-      if (env_int("MVD_XBLK", 0) > 0) c->xt_blocks[mode] = std::min(c->xt_blocks[mode], env_int("MVD_XBLK", 0));
       if (c->xt_blocks[mode] <= 0) { snprintf(c->err, sizeof(c->err), "x pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
     }
     const long long ntiles = (a.nrows + a.rows_per_cta - 1) / a.rows_per_cta;

@@ -424,13 +424,9 @@ struct Launch {
 
   static cudaError_t init() {
     const int big = 200 * 1024;
-    const char* cs = getenv("MVD_CARVEOUT");
-    const int carve = cs ? atoi(cs) : -1;
     cudaError_t e;
 #define MVD_SET(k) \
   e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, big); \
-  if (e != cudaSuccess) return e; \
-  if (carve >= 0) e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, carve); \
   if (e != cudaSuccess) return e;
     MVD_SET((strided_fft_kernel<A, B, -1>));
     MVD_SET((strided_fft_kernel<A, B, 1>));

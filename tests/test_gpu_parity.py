@@ -545,3 +545,15 @@ def test_every_compiled_length_on_every_axis(mvd, axis):
         d.close()
         tested += 1
     assert tested >= 50
+
+
+def test_register_staged_fallback_kernels_match_too(mvd, tiny, monkeypatch):
+    """The register-staged passes (pass_kernels.cuh) stay as the fallback when a pencil does not fit
+    the TMA-staged tiles; MVD_XTMA/YTMA/ZTMA=0 selects them.  Same parity bar."""
+    for k in ("MVD_XTMA", "MVD_YTMA", "MVD_ZTMA"):
+        monkeypatch.setenv(k, "0")
+    for variant in ("osem", "efficient"):
+        g, _ = gpu_checkpoints(mvd, tiny, variant, "auto", (1, 3))
+        o, _ = oracle_checkpoints(tiny, variant, "auto", (1, 3))
+        check(g[1], o[1], 1, "fallback %s" % variant)
+        check(g[3], o[3], 3, "fallback %s" % variant)
