@@ -557,3 +557,29 @@ def test_register_staged_fallback_kernels_match_too(mvd, tiny, monkeypatch):
         o, _ = oracle_checkpoints(tiny, variant, "auto", (1, 3))
         check(g[1], o[1], 1, "fallback %s" % variant)
         check(g[3], o[3], 3, "fallback %s" % variant)
+
+
+def test_views_not_16_byte_aligned(mvd):
+    """Borrowed views (and weights) only need float alignment: rows that cannot be staged by 16-byte
+    bulk copies take the plain-load path inside the same kernel."""
+    import torch
+    p = mvd_synth.make_tiny_asymmetric(dims=(24, 20, 18), psf_dims=(5, 7, 9), n_views=2)
+    n = p.views[0].size
+    views, wts = [], []
+    ws = _partial_overlap_weights(p.views[0].shape, 2)
+    for v, w in zip(p.views, ws):
+        big = torch.zeros(n + 3, dtype=torch.float32, device="cuda")
+        big[1:1 + n] = torch.from_numpy(v.ravel()).cuda()
+        views.append(big[1:1 + n].view(p.views[0].shape))
+        bw = torch.zeros(n + 3, dtype=torch.float32, device="cuda")
+        bw[3:3 + n] = torch.from_numpy(w.astype(np.float32).ravel()).cuda()
+        wts.append(bw[3:3 + n].view(p.views[0].shape))
+        assert views[-1].data_ptr() % 16 == 4 and wts[-1].data_ptr() % 16 == 12
+    w32 = [w.astype(np.float32).astype(np.float64) for w in ws]
+    for kw, okw in (({}, {}), ({"weights": wts}, {"weights": w32})):
+        d = mvd.Deconvolver(views, p.psfs, variant="osem", **kw)
+        d.iterate(3)
+        o = O.Oracle(p.views, p.psfs, "osem", **okw)
+        o.iterate(3)
+        check(d.get_estimate_host(), o.psi, 3, "misaligned views %s" % list(kw))
+        d.close()
