@@ -706,7 +706,9 @@ mvd_status build_spectrum(mvd_ctx* c, const double* kern, Dims3 K, float2* spec)
   return MVD_OK;
 }
 
-mvd_status precompute(mvd_ctx* c, const float* const* psfs_host) {
+// shared_kern: the back-projectors K_v of an earlier context of the same problem (blocked mode: one
+// context per block shape, same PSFs), V * psf_stride doubles on the device; NULL -> compute them
+mvd_status precompute(mvd_ctx* c, const float* const* psfs_host, const double* shared_kern) {
   const Plan& P = c->P;
   // twiddle tables, generated in double
   {
@@ -740,7 +742,11 @@ mvd_status precompute(mvd_ctx* c, const float* const* psfs_host) {
     MVD_CK(cudaStreamSynchronize(c->stream), "PSF upload");   // the staging buffer is reused
   }
   // back-projectors K_v (O3)
-  if (P.kmode == MVD_KERNEL_COMPOUND) {
+  if (shared_kern) {
+    MVD_CK(cudaMemcpyAsync(c->kern(0), shared_kern, sizeof(double) * P.psf_stride * P.V, cudaMemcpyDeviceToDevice, c->stream),
+           "back-projector copy");
+  }
+  if (!shared_kern && P.kmode == MVD_KERNEL_COMPOUND) {
     for (int w = 0; w < P.V; ++w) {
       const Dims3 K = P.K[w];
       const long long tot = (long long)(2 * K.x - 1) * (2 * K.y - 1) * (2 * K.z - 1);
@@ -750,7 +756,7 @@ mvd_status precompute(mvd_ctx* c, const float* const* psfs_host) {
     }
   }
   for (int v = 0; v < P.V; ++v) {
-    if (!c->is_local[v]) continue;
+    if (!c->is_local[v] || shared_kern) continue;
     const Dims3 K = P.K[v];
     const long long tot = (long long)K.x * K.y * K.z;
     const unsigned g256 = (unsigned)((tot + 255) / 256), g128 = (unsigned)((tot + 31) / 32);   // corr: one block of 256 threads per 32 taps
@@ -858,9 +864,19 @@ mvd_status mvd_plan_dims(int n_views, const int dims[3], const int (*psf_dims)[3
   return MVD_OK;
 }
 
+static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* views, const int dims[3],
+                              const float* const* psfs, const int (*psf_dims)[3], mvd_variant variant,
+                              const mvd_options* opt_in, const double* shared_kern);
+
 mvd_status mvd_create(mvd_ctx** out, int n_views, const float* const* views, const int dims[3],
                       const float* const* psfs, const int (*psf_dims)[3], mvd_variant variant,
                       const mvd_options* opt_in) {
+  return create_impl(out, n_views, views, dims, psfs, psf_dims, variant, opt_in, nullptr);
+}
+
+static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* views, const int dims[3],
+                              const float* const* psfs, const int (*psf_dims)[3], mvd_variant variant,
+                              const mvd_options* opt_in, const double* shared_kern) {
   if (!out) return MVD_ERR_INVALID_ARG;
   *out = nullptr;
   if (!views || !psfs || !dims || !psf_dims || !opt_in) return MVD_ERR_INVALID_ARG;
@@ -928,7 +944,7 @@ mvd_status mvd_create(mvd_ctx** out, int n_views, const float* const* views, con
     return MVD_ERR_CUDA;
   }
 
-  s = precompute(c, psfs);
+  s = precompute(c, psfs, shared_kern);
   if (s == MVD_OK && opt->views_ready &&
       c->fail(cudaStreamWaitEvent(c->stream, reinterpret_cast<cudaEvent_t>(opt->views_ready), 0), "views_ready"))
     s = MVD_ERR_CUDA;
@@ -1181,7 +1197,8 @@ struct BlockedLayout {
   size_t max_ext = 0;          // voxels of the largest extended block
   size_t ctx_bytes = 0;        // largest context workspace over the distinct extended shapes
   std::vector<std::array<int, 3>> shapes;
-  size_t off_scal = 0, off_views = 0, off_psi0 = 0, off_est = 0, off_ctx = 0, total = 0;
+  size_t off_scal = 0, off_views = 0, off_psi0 = 0, off_est = 0, off_kern = 0, off_ctx = 0, total = 0;
+  size_t kern_bytes = 0;       // back-projectors shared by the contexts of all block shapes
 };
 
 mvd_status blocked_layout(BlockedLayout& L, int n_views, const int dims[3], const int (*psf_dims)[3],
@@ -1217,6 +1234,13 @@ mvd_status blocked_layout(BlockedLayout& L, int n_views, const int dims[3], cons
   L.off_views = take(align_up(L.max_ext * sizeof(float), 256) * n_views);
   L.off_psi0 = take(L.max_ext * sizeof(float));
   L.off_est = take(L.max_ext * sizeof(float));
+  {
+    size_t kmax = 0;
+    for (int v = 0; v < n_views; ++v)
+      kmax = std::max(kmax, (size_t)psf_dims[v][0] * psf_dims[v][1] * psf_dims[v][2]);
+    L.kern_bytes = align_up(kmax, 32) * sizeof(double) * n_views;   // = psf_stride * V of every context
+  }
+  L.off_kern = take(L.kern_bytes);
   L.off_ctx = take(L.ctx_bytes);
   L.total = off;
   return MVD_OK;
@@ -1271,6 +1295,8 @@ extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* vi
   ++launches;
   if (cudaGetLastError() != cudaSuccess) return MVD_ERR_CUDA;
 
+  double* shared_kern = reinterpret_cast<double*>(ws + L.off_kern);
+  bool have_kern = false;
   for (const auto& shape : L.shapes) {
     const int d[3] = {shape[0], shape[1], shape[2]};
     mvd_options o = *opt;
@@ -1279,8 +1305,16 @@ extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* vi
     o.workspace = ws + L.off_ctx;
     o.workspace_bytes = L.ctx_bytes;
     mvd_ctx* c = nullptr;
-    s = mvd_create(&c, n_views, bviews.data(), d, psfs, psf_dims, variant, &o);
+    s = create_impl(&c, n_views, bviews.data(), d, psfs, psf_dims, variant, &o, have_kern ? shared_kern : nullptr);
     if (s != MVD_OK) return s;
+    if (!have_kern) {   // the back-projectors depend on the PSFs only: computed once, reused by the other shapes
+      if (sizeof(double) * c->P.psf_stride * c->P.V != L.kern_bytes ||
+          cudaMemcpyAsync(shared_kern, c->kern(0), L.kern_bytes, cudaMemcpyDeviceToDevice, st) != cudaSuccess) {
+        mvd_destroy(c);
+        return MVD_ERR_CUDA;
+      }
+      have_kern = true;
+    }
     const Dims3 E{d[0], d[1], d[2]};
     const long long ext = (long long)d[0] * d[1] * d[2];
     const unsigned grid = (unsigned)std::min<long long>((ext + 255) / 256, 1184 * 8);
