@@ -150,11 +150,15 @@ def hbm_peak():
 
 def ncu_traffic(kernel_class, k):
     """dram bytes per launch of the class from the committed ncu --set full capture, or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    p = os.path.join(ROOT, "profiles", "r01e_traffic.csv")
     try:
-        return json.load(open(p))["config%d" % k][kernel_class]
+        for line in open(p).read().splitlines()[1:]:
+            cfg, cls, val = line.split(",")
+            if int(cfg) == k and cls == kernel_class:
+                return int(val)
     except Exception:
-        return None
+        pass
+    return None
 
 
 # ------------------------------------------------------------------------------------------
