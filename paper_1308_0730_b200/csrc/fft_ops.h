@@ -12,6 +12,9 @@ namespace mvd {
 #define MVD_TMA_TILE 8
 #endif
 constexpr int kTmaTileHost = MVD_TMA_TILE;   // == kTmaTile of pass_tma.cuh
+// tile width of the TMA-staged y pass for pencil length M: pencils too long for two resident CTAs
+// get 12-wide tiles (two stages still fit, 1.5x the threads per CTA; config 5: 1227 -> 1003 us)
+__host__ __device__ constexpr int strided_tma_tile(int M) { return (M > 880 && M <= 1140) ? 12 : kTmaTileHost; }
 
 // ---- TMA-staged strided pass (pass_tma.cuh): persistent CTAs, tiles of T contiguous complex
 //      elements x the whole pencil, loaded by tensor copies with zero fill beyond n_in ----------

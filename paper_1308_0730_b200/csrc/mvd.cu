@@ -248,7 +248,7 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
       }
       if (best == 0) best = 4;
       (void)force;
-      best = kTmaTileHost;
+      best = zconv ? kTmaTileHost : strided_tma_tile(l->M);
       const int items = best * ab * (zconv ? 2 : 1);   // the z tile is 8 x by 2 rows
       const int rounds = (items + l->max_threads - 1) / l->max_threads;
       *T_out = best;
@@ -263,7 +263,7 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
       // two tile stages whenever they fit (one stage with more CTAs per SM measured slower on config 5)
       const int nbox = (P.ly->M + 255) / 256;
       const int boxr = ((P.ly->M + nbox - 1) / nbox + 3) / 4 * 4;
-      P.ynst = P.ly->strided_tma_smem(kTmaTileHost, boxr, nbox, 2) <= 218 * 1024 ? 2 : 1;
+      P.ynst = P.ly->strided_tma_smem(strided_tma_tile(P.ly->M), boxr, nbox, 2) <= 218 * 1024 ? 2 : 1;
       const int force = env_int("MVD_YNST", 0);
       if (force == 1 || force == 2) P.ynst = force;
       const int nbz = (P.lz->M + 255) / 256;

@@ -299,7 +299,7 @@ __global__ void __launch_bounds__(PassCfg<A, B>::MAX_THREADS)
 strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
   constexpr int M = A * B;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  constexpr int T = kTmaTile;
+  constexpr int T = strided_tma_tile(M);
   const int NR = p.boxr * p.nbox;
   const int nst = p.nst;                                          // tile stages: 1 or 2
   float2* buf = reinterpret_cast<float2*>(smem_raw);            // [nst][NR][T]
