@@ -117,6 +117,13 @@ MVD_API size_t mvd_workspace_size(int n_views, const int dims[3], const int (*ps
 MVD_API mvd_status mvd_plan_dims(int n_views, const int dims[3], const int (*psf_dims)[3],
                          const mvd_options* opt, int fft_dims_out[3]);
 
+/* Quality of the current estimate against a caller-supplied reference volume (DEVICE pointer, N voxels): the two
+ * measures the paper reports, the average absolute difference and the cross-correlation
+ * (Pearson coefficient, L48).  fp64 accumulation in warp-shuffle reductions; synchronises the stream.
+ * Either output pointer may be NULL. */
+MVD_API mvd_status mvd_compare(mvd_ctx* ctx, const float* ref_device, double* average_difference,
+                               double* cross_correlation);
+
 /* View-parallel form of the combined variants ("all view contributions can be computed at the same
  * time"; eq. 70 / 104 with the root of eq. 44).  Each rank owns some views and the same psi:
  *   mvd_partial_product : acc <- prod over the context's own views of max(f_v, 0) (f_v itself if literal_product),

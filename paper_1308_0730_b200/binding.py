@@ -25,7 +25,7 @@ SYMBOLS = (
     "mvd_get_estimate", "mvd_set_estimate", "mvd_get_stats", "mvd_get_back_projector", "mvd_convolve",
     "mvd_launch_count", "mvd_profile", "mvd_profile_read", "mvd_kernel_class_name", "mvd_blocked_workspace_size", "mvd_deconvolve_blocked", "mvd_destroy",
     "mvd_status_string", "mvd_last_error",
-    "mvd_partial_product", "mvd_get_product", "mvd_apply_product", "mvd_reduce_scratch_bytes", "mvd_reduce_sum",
+    "mvd_compare", "mvd_partial_product", "mvd_get_product", "mvd_apply_product", "mvd_reduce_scratch_bytes", "mvd_reduce_sum",
 )
 
 
@@ -109,6 +109,8 @@ def load_library():
     lib.mvd_status_string.restype = C.c_char_p
     lib.mvd_last_error.argtypes = [vp]
     lib.mvd_last_error.restype = C.c_char_p
+    lib.mvd_compare.argtypes = [vp, vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.mvd_compare.restype = C.c_int
     lib.mvd_partial_product.argtypes = [vp]
     lib.mvd_partial_product.restype = C.c_int
     lib.mvd_get_product.argtypes = [vp, C.POINTER(vp)]
@@ -267,6 +269,15 @@ class Deconvolver:
     def iterate(self, n=1):
         with self._torch.cuda.device(self.device):
             _check(self._lib.mvd_iterate(self._ctx, int(n)), self._ctx, "mvd_iterate")
+
+    def compare(self, ref):
+        """mvd_compare: (average absolute difference, cross-correlation) of psi against a reference volume."""
+        r = ref.to(device=self.device, dtype=self._torch.float32).contiguous()
+        self.stream.wait_stream(self._torch.cuda.current_stream(self.device))
+        a, x = C.c_double(), C.c_double()
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.mvd_compare(self._ctx, r.data_ptr(), C.byref(a), C.byref(x)), self._ctx, "mvd_compare")
+        return a.value, x.value
 
     def partial_product(self):
         """mvd_partial_product: acc <- product over this context's views of max(f_v, 0), psi unchanged."""

@@ -199,6 +199,28 @@ __global__ void paste_block_kernel(const float* __restrict__ src, Dims3 E, Dims3
   }
 }
 
+// per-block partial sums for the quality metrics against a reference (L127, L48):
+// out[6*b + {0..5}] = sum |a-r|, sum a, sum r, sum a^2, sum r^2, sum a*r
+__global__ void __launch_bounds__(256) compare_kernel(const float* __restrict__ a, const float* __restrict__ r,
+                                                      long long n, double* __restrict__ out) {
+  __shared__ double red[32];
+  double s[6] = {0, 0, 0, 0, 0, 0};
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const double x = a[i], y = r[i];
+    s[0] += fabs(x - y);
+    s[1] += x;
+    s[2] += y;
+    s[3] += x * x;
+    s[4] += y * y;
+    s[5] += x * y;
+  }
+  for (int k = 0; k < 6; ++k) {
+    const double t = block_sum(s[k], red);
+    if (threadIdx.x == 0) out[6 * (size_t)blockIdx.x + k] = t;
+  }
+}
+
 __global__ void fill_value_kernel(float* __restrict__ a, long long n, float value) {
   const long long stride = (long long)gridDim.x * blockDim.x;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) a[i] = value;

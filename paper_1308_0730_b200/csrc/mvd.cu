@@ -93,7 +93,7 @@ struct Plan {
   // workspace offsets (bytes)
   size_t off_twx = 0, off_twy = 0, off_twz = 0, off_psi = 0, off_acc = 0, off_w = 0, off_w0 = 0,
          off_spec = 0, off_psf = 0, off_kern = 0, off_auto = 0, off_stage = 0, off_partials = 0,
-         off_scalars = 0, total = 0;
+         off_scalars = 0, off_cmp = 0, total = 0;
   size_t psf_stride = 0, auto_stride = 0;   // elements (doubles) per view
   int sum_blocks = 0;
 };
@@ -325,6 +325,7 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
   P.sum_blocks = 1184;   // 148 SMs x 8
   P.off_partials = take(sizeof(double) * 2 * (size_t)std::max(P.nctax, P.sum_blocks));
   P.off_scalars = take(sizeof(double) * (size_t)(P.V + 8));
+  P.off_cmp = take(sizeof(double) * (6 * 192 + 8));   // mvd_compare partials
   P.total = o;
   return MVD_OK;
 }
@@ -988,6 +989,29 @@ mvd_status mvd_iterate(mvd_ctx* c, int n) {
   for (int i = 0; i < n; ++i) {
     MVD_TRY(iteration_body(c));
     ++c->iters;
+  }
+  return MVD_OK;
+}
+
+mvd_status mvd_compare(mvd_ctx* c, const float* ref, double* avg_diff, double* xcorr) {
+  if (!c || !ref) return MVD_ERR_INVALID_ARG;
+  if (c->broken) return MVD_ERR_STATE;
+  const Plan& P = c->P;
+  const int nb = 192;
+  double* part = reinterpret_cast<double*>(c->ws + P.off_cmp);
+  compare_kernel<<<nb, 256, 0, c->stream>>>(c->psi(), ref, P.nvox, part);
+  MVD_CK(cudaGetLastError(), "compare_kernel");
+  final_sum_kernel<<<1, 256, 0, c->stream>>>(part, nb, 6, part + 6 * nb);
+  MVD_CK(cudaGetLastError(), "final_sum_kernel");
+  c->launches += 2;
+  double h[6];
+  MVD_CK(cudaMemcpyAsync(h, part + 6 * nb, sizeof(h), cudaMemcpyDeviceToHost, c->stream), "compare copy");
+  MVD_CK(cudaStreamSynchronize(c->stream), "compare copy");
+  const double n = (double)P.nvox;
+  if (avg_diff) *avg_diff = h[0] / n;
+  if (xcorr) {
+    const double cov = h[5] - h[1] * h[2] / n, va = h[3] - h[1] * h[1] / n, vr = h[4] - h[2] * h[2] / n;
+    *xcorr = (va > 0.0 && vr > 0.0) ? cov / sqrt(va * vr) : 0.0;
   }
   return MVD_OK;
 }

@@ -583,3 +583,21 @@ def test_views_not_16_byte_aligned(mvd):
         o.iterate(3)
         check(d.get_estimate_host(), o.psi, 3, "misaligned views %s" % list(kw))
         d.close()
+
+
+def test_quality_metrics_against_a_reference(mvd):
+    """mvd_compare: average difference (L127) and cross-correlation (L48) of psi against the ground
+    truth, against the same measures computed by the oracle module on the same estimate."""
+    import torch
+    p = mvd_synth.make_problem(1, dims=(40, 36, 32), psf_dims=(7, 7, 15))
+    d = mvd.Deconvolver(to_dev(p.views), p.psfs, variant="osem")
+    d.iterate(3)
+    st0 = d.get_stats()
+    psi = d.get_estimate_host().astype(np.float64)
+    ad, cc = d.compare(torch.from_numpy(p.gt.astype(np.float32)).cuda())
+    gt32 = p.gt.astype(np.float32).astype(np.float64)
+    assert ad == pytest.approx(O.average_difference(psi, gt32), rel=1e-9)
+    assert cc == pytest.approx(O.cross_correlation(psi, gt32), rel=1e-9)
+    assert 0.0 < cc <= 1.0
+    assert d.get_stats() == st0                       # the update statistics survive a comparison
+    d.close()
