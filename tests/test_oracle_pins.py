@@ -363,3 +363,14 @@ def test_normalise_weights_never_increases_and_caps_the_sum():
             assert np.array_equal(a[untouched], b[untouched])
         capped = ~untouched
         assert np.allclose(tot[capped], cap)
+
+
+def test_quality_metrics_are_the_library_definitions():
+    """L48 cross-correlation = Pearson coefficient (numpy.corrcoef); L127 average difference = mean |a-b|."""
+    rng = np.random.default_rng(4)
+    a, b = rng.random((5, 6, 7)), rng.random((5, 6, 7))
+    assert O.cross_correlation(a, b) == pytest.approx(np.corrcoef(a.ravel(), b.ravel())[0, 1], rel=1e-12)
+    assert O.cross_correlation(a, 3 * a + 2) == pytest.approx(1.0, rel=1e-12)
+    assert O.cross_correlation(a, -a) == pytest.approx(-1.0, rel=1e-12)
+    assert O.average_difference(a, a + 0.25) == pytest.approx(0.25, rel=1e-12)
+    assert O.average_difference(a, b) == pytest.approx(np.mean(np.abs(a - b)), rel=1e-14)
