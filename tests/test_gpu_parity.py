@@ -601,3 +601,13 @@ def test_quality_metrics_against_a_reference(mvd):
     assert 0.0 < cc <= 1.0
     assert d.get_stats() == st0                       # the update statistics survive a comparison
     d.close()
+
+
+def test_blocked_config2_size_shares_back_projectors(mvd, config2):
+    """128^3, PSF 17x17x35, 64^3 blocks + halo: 8 blocks of several extended shapes (one context per
+    shape, the compound kernels computed once and shared) against the blocked oracle."""
+    block = (64, 64, 64)
+    got, launches = mvd.deconvolve_blocked(to_dev(config2.views), config2.psfs, block, 3, variant="osem")
+    ref = O.deconvolve_blocked(config2.views, config2.psfs, block[::-1], "osem", 3)
+    check(got.cpu().numpy(), ref, 3, "blocked config 2")
+    assert launches > 8 * 3 * 3 * 8
