@@ -138,15 +138,16 @@ MVD_DEV float2 cscale(float c, float2 s) {
   return r;
 }
 #endif
-// a * b and a * conj(b) as  a.x * (b.x, +-b.y) + a.y * (-+b.y, b.x): two packed instructions and one
-// sign flip; the order of operations is fixed, so every kernel rounds a product the same way
+// a * b and a * conj(b): one packed multiply a.x * (b.x, b.y) and two scalar FMAs for the a.y terms
+// (no sign flip, no constant pair to build); the order of operations is fixed, so every kernel
+// rounds a product the same way
 MVD_DEV float2 cmul(float2 a, float2 b) {
   const float2 t = mul2(a.x, a.x, b.x, b.y);
-  return fma2(a.y, a.y, -b.y, b.x, t.x, t.y);
+  return make_float2(MVD_FMA(-a.y, b.y, t.x), MVD_FMA(a.y, b.x, t.y));
 }
-MVD_DEV float2 cmul_conj(float2 a, float2 b) {   // a * conj(b)
+MVD_DEV float2 cmul_conj(float2 a, float2 b) {   // a * conj(b) = (a.x b.x + a.y b.y, a.y b.x - a.x b.y)
   const float2 t = mul2(a.y, a.y, b.y, b.x);
-  return fma2(a.x, a.x, b.x, -b.y, t.x, t.y);
+  return make_float2(MVD_FMA(a.x, b.x, t.x), MVD_FMA(-a.x, b.y, t.y));
 }
 // a * w for a table entry e = (w.x, w.y, -w.y, w.x): two packed instructions, no sign flip
 MVD_DEV float2 cmul_tab(float2 a, float4 e) {
@@ -170,8 +171,8 @@ MVD_DEV float2 cmul_root(float2 a) {
     constexpr cdouble w = ce_root(k, N);
     constexpr float c = float(w.re);
     constexpr float s = float(DIR > 0 ? w.im : -w.im);
-    const float2 t = mul2(a.x, a.x, c, s);
-    return fma2(a.y, a.y, -s, c, t.x, t.y);
+    const float2 t = mul2(a.x, a.y, c, c);            // packed multiply by the broadcast immediate c
+    return make_float2(MVD_FMA(-s, a.y, t.x), MVD_FMA(s, a.x, t.y));
   }
 }
 
