@@ -150,7 +150,7 @@ def hbm_peak():
 
 def ncu_traffic(kernel_class, k):
     """dram bytes per launch of the class from the committed ncu --set full capture, or None."""
-    p = os.path.join(ROOT, "profiles", "r01e_traffic.csv")
+    p = os.path.join(ROOT, "profiles", "r01f_traffic.csv")
     try:
         for line in open(p).read().splitlines()[1:]:
             cfg, cls, val = line.split(",")

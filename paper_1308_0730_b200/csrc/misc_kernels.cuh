@@ -123,7 +123,7 @@ __global__ void __launch_bounds__(256) corr_crop_mul_kernel(const double* __rest
   const long long jj = live ? j : tot - 1;
   const int jx = int(jj % K.x), jy = int((jj / K.x) % K.y), jz = int(jj / ((long long)K.x * K.y));
   const int ox = (Gd.x - 1) / 2 + jx, oy = (Gd.y - 1) / 2 + jy, oz = (Gd.z - 1) / 2 + jz;
-  double acc = 0.0;
+  double acc = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
   const int nrows = K.z * K.y;
   for (int r = warp; r < nrows; r += 8) {
     const int uz = r / K.y, uy = r - uz * K.y;
@@ -131,11 +131,18 @@ __global__ void __launch_bounds__(256) corr_crop_mul_kernel(const double* __rest
     if (gz < 0 || gz >= Gd.z || gy < 0 || gy >= Gd.y) continue;
     const double* pv = Pv + ((long long)(K.z - 1 - uz) * K.y + (K.y - 1 - uy)) * K.x;
     const double* g = G + ((long long)gz * Gd.y + gy) * Gd.x;
-    for (int ux = 0; ux < K.x; ++ux) {
-      const int gx = ox - ux;
-      if (gx >= 0 && gx < Gd.x) acc += pv[K.x - 1 - ux] * g[gx];
+    // valid ux: 0 <= ox - ux < Gd.x; four independent partial sums hide the fp64 FMA latency
+    const int u0 = max(0, ox - Gd.x + 1), u1 = min(K.x - 1, ox);
+    int ux = u0;
+    for (; ux + 3 <= u1; ux += 4) {
+      acc += pv[K.x - 1 - ux] * g[ox - ux];
+      acc1 += pv[K.x - 2 - ux] * g[ox - ux - 1];
+      acc2 += pv[K.x - 3 - ux] * g[ox - ux - 2];
+      acc3 += pv[K.x - 4 - ux] * g[ox - ux - 3];
     }
+    for (; ux <= u1; ++ux) acc += pv[K.x - 1 - ux] * g[ox - ux];
   }
+  acc += acc1 + acc2 + acc3;
   red[warp][lane] = acc;
   __syncthreads();
   if (warp == 0 && live) {
