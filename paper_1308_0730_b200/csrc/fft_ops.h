@@ -12,9 +12,10 @@ namespace mvd {
 #define MVD_TMA_TILE 8
 #endif
 constexpr int kTmaTileHost = MVD_TMA_TILE;   // == kTmaTile of pass_tma.cuh
-// tile width of the TMA-staged y pass for pencil length M: pencils too long for two resident CTAs
-// get 12-wide tiles (two stages still fit, 1.5x the threads per CTA; config 5: 1227 -> 1003 us)
-__host__ __device__ constexpr int strided_tma_tile(int M) { return (M > 880 && M <= 1140) ? 12 : kTmaTileHost; }
+// tile width of the TMA-staged y pass for pencil length M: 8 for short pencils (three CTAs per SM with two
+// stages), 12 for 501-1140 points (measured: config 4 115 -> 111 us, config 5 1227 -> 1003 us), 8 beyond
+// (two 12-wide stages no longer fit)
+__host__ __device__ constexpr int strided_tma_tile(int M) { return (M > 500 && M <= 1140) ? 12 : kTmaTileHost; }
 
 // ---- TMA-staged strided pass (pass_tma.cuh): persistent CTAs, tiles of T contiguous complex
 //      elements x the whole pencil, loaded by tensor copies with zero fill beyond n_in ----------
