@@ -193,13 +193,10 @@ MVD_DEV void bfly4(float2& a, float2& b, float2& c, float2& d) {
   a = cadd(s0, s1);
   c = csub(s0, s1);
   // b = d0 + DIR*i*d1, d = d0 - DIR*i*d1 with i*d1 = (-d1.y, d1.x)
-  if constexpr (DIR > 0) {
-    b = make_float2(d0.x - d1.y, d0.y + d1.x);
-    d = make_float2(d0.x + d1.y, d0.y - d1.x);
-  } else {
-    b = make_float2(d0.x + d1.y, d0.y - d1.x);
-    d = make_float2(d0.x - d1.y, d0.y + d1.x);
-  }
+  // b = d0 + DIR*i*d1, d = d0 - DIR*i*d1 with i*d1 = (-d1.y, d1.x): swapped operand, sign pair constant
+  constexpr float sg = DIR > 0 ? 1.f : -1.f;
+  b = fma2(d1.y, d1.x, -sg, sg, d0.x, d0.y);
+  d = fma2(d1.y, d1.x, sg, -sg, d0.x, d0.y);
 }
 
 // odd prime P: pairs (m, P-m).  X_j = a_j + i*DIR*b_j, X_{P-j} = a_j - i*DIR*b_j with
@@ -229,13 +226,9 @@ MVD_DEV void bfly_odd(float2 (&x)[P]) {
       else b = caxpy(sn, d[m - 1], b);
     });
     // x[j] = a + i*DIR*b, x[P-j] = a - i*DIR*b with i*b = (-b.y, b.x)
-    if constexpr (DIR > 0) {
-      x[j] = make_float2(a.x - b.y, a.y + b.x);
-      x[P - j] = make_float2(a.x + b.y, a.y - b.x);
-    } else {
-      x[j] = make_float2(a.x + b.y, a.y - b.x);
-      x[P - j] = make_float2(a.x - b.y, a.y + b.x);
-    }
+    constexpr float sg = DIR > 0 ? 1.f : -1.f;
+    x[j] = fma2(b.y, b.x, -sg, sg, a.x, a.y);
+    x[P - j] = fma2(b.y, b.x, sg, -sg, a.x, a.y);
   });
 }
 
