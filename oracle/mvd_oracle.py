@@ -23,9 +23,12 @@ Arrays are numpy, shape (Nz, Ny, Nx), x fastest.  All arithmetic is float64.
 Pins (tests/test_oracle_pins.py): P1 brute force == FFT, P2 V=1 == classical RL, P3 flux
 identity (eq. 52-55), P4 fixed point (L306), P5 identical views (L847), P6 delta PSF (L851),
 P7 Gaussian closed form of eq. 105, P8 monotone likelihood (eq. 39-43), P9 ordering (L807-809),
-hand-computed worked example (tests/golden/rl_1d_worked_example.txt).
+hand-computed worked example (tests/golden/rl_1d_worked_example.txt); deconvolve_blocked: exact
+equality with the whole-volume result when the halo covers the dependence radius (2r per
+view-update), delta PSF with halo 0, and a negative control with halo r.
 Parity unpinned by the paper (shared definitions only, R2/R4/R13): eps / psi_floor clamps,
-psi0 = mean over all views, the OSEM=compound default, the block halo rule.
+psi0 = mean over all views, the OSEM=compound default, the halo WIDTH r of the block mode
+(the block mechanics themselves are pinned as above).
 """
 from __future__ import annotations
 
@@ -229,19 +232,26 @@ class Oracle:
     def factor(self, v):
         return rl_factor(self.psi, self.views[v], self.psfs[v], self.kernels[v], self.eps, self.backend)
 
+    def view_update(self, v):
+        """One sequential update with view v (one line of eq. 109-112): psi <- max(psi f_v, floor)."""
+        if self.variant != "osem":
+            raise ValueError("view_update is the sequential (OSEM) step")
+        f = self.factor(v)
+        if self.weights is not None:
+            # section 12 (L897): the weight 0..1 of a pixel is "the fraction of change
+            # suggested by a Lucy-Richardson update step that will be applied":
+            # psi*f = psi + (psi*f - psi)  ->  psi + w*(psi*f - psi) = psi*(1 + w*(f - 1))
+            f = 1.0 + self.weights[v] * (f - 1.0)
+        self._commit(np.maximum(self.psi * f, self.psi_floor))
+        return self.psi
+
     def iterate(self, n=1):
         nv = len(self.views)
         for _ in range(n):
             if self.variant == "osem":
                 # eq. 109-112 / 114-117: psi is updated after every view, index order (R11)
                 for v in range(nv):
-                    f = self.factor(v)
-                    if self.weights is not None:
-                        # section 12 (L897): the weight 0..1 of a pixel is "the fraction of change
-                        # suggested by a Lucy-Richardson update step that will be applied":
-                        # psi*f = psi + (psi*f - psi)  ->  psi + w*(psi*f - psi) = psi*(1 + w*(f - 1))
-                        f = 1.0 + self.weights[v] * (f - 1.0)
-                    self._commit(np.maximum(self.psi * f, self.psi_floor))
+                    self.view_update(v)
             else:
                 # eq. 70 / 104: every f_v from the same psi^r, multiplicative combination
                 prod = np.ones_like(self.psi)
@@ -294,13 +304,6 @@ def normalise_weights(weights, max_sum=1.0):
 # --------------------------------------------------------------------------------------
 # quality metrics the paper uses (L127 average difference, L48 cross-correlation)
 # --------------------------------------------------------------------------------------
-def log_likelihood(psi, psi_star):
-    """eq. 39 (L433): L(psi; psi*) = -sum psi* log(psi*/psi)."""
-    psi = np.asarray(psi, dtype=np.float64)
-    psi_star = np.asarray(psi_star, dtype=np.float64)
-    return float(-(psi_star * np.log(psi_star / psi)).sum())
-
-
 def average_difference(psi, ref):
     return float(np.abs(np.asarray(psi, np.float64) - np.asarray(ref, np.float64)).mean())
 

@@ -292,6 +292,84 @@ def test_blocked_is_close_to_whole_in_block_interiors():
     assert blk.shape == whole.shape and np.isfinite(blk).all()
 
 
+def _dependence_exact_case(n_views, seed):
+    """Asymmetric PSFs of different half-size per axis, a volume that the blocks tile raggedly."""
+    rng = np.random.default_rng([13080730, 600 + seed])
+    shape = (23, 19, 26)                                        # (Nz, Ny, Nx)
+    box = (5, 3, 7)                                             # (Kx, Ky, Kz): r = (2, 1, 3)
+    psfs = [mvd_synth.random_psf(rng, box) for _ in range(n_views)]
+    views = [rng.random(shape) * 40 + 5 for _ in range(n_views)]
+    return views, psfs, (3, 1, 2)                               # r in (z, y, x) order
+
+
+@pytest.mark.parametrize("block_zyx", [(8, 7, 9), (23, 6, 26), (5, 19, 4), (12, 10, 13)])
+def test_blocked_equals_whole_exactly_when_halo_covers_the_dependence_radius(block_zyx):
+    """R13 / L943.  One view-update reads psi within 2r of a voxel (b = psi*P needs r, f = q*K another
+    r) and psi^0 is the same constant on both sides, so with V = 1, one iteration and halo = 2r the
+    block-wise result IS the whole-volume result at every voxel (clipping the halo at a volume face
+    is the same zero extension).  A +-1 error in the halo clip or the paste offset fails this."""
+    views, psfs, r = _dependence_exact_case(1, 0)
+    whole = O.deconvolve(views, psfs, "osem", 1)
+    blk = O.deconvolve_blocked(views, psfs, block_zyx, "osem", 1, halo_zyx=tuple(2 * x for x in r))
+    assert np.abs(blk - whole).max() / whole.max() < 1e-12
+    # all three schedules coincide for one view (P2), blocked too
+    blk2 = O.deconvolve_blocked(views, psfs, block_zyx, "efficient", 1, halo_zyx=tuple(2 * x for x in r))
+    assert np.abs(blk2 - whole).max() / whole.max() < 1e-12
+
+
+def test_blocked_exact_for_several_views_and_iterations_with_the_full_radius():
+    """Sequential updates chain: V views x n iterations read psi within 2r*V*n; halo of that size is exact."""
+    views, psfs, r = _dependence_exact_case(2, 1)
+    whole = O.deconvolve(views, psfs, "osem", 1, kernel_mode="plain")
+    halo = tuple(2 * x * 2 for x in r)
+    blk = O.deconvolve_blocked(views, psfs, (8, 7, 9), "osem", 1, halo_zyx=halo, kernel_mode="plain")
+    assert np.abs(blk - whole).max() / whole.max() < 1e-12
+
+
+def test_blocked_with_too_small_a_halo_differs_at_block_borders_only():
+    """Negative control: halo = r (the BASELINE rule) is NOT exact: voxels within r of an inner block
+    border see b computed from a zero-extended psi.  Voxels >= 2r - halo = r inside their block are exact."""
+    views, psfs, r = _dependence_exact_case(1, 2)
+    whole = O.deconvolve(views, psfs, "osem", 1)
+    block = (12, 10, 13)
+    blk = O.deconvolve_blocked(views, psfs, block, "osem", 1, halo_zyx=r)
+    rel = np.abs(blk - whole) / whole.max()
+    assert rel.max() > 1e-4                                      # the borders do differ
+    exact = np.zeros(whole.shape, bool)                          # distance >= r from every inner block border
+    for (z0, z1), (y0, y1), (x0, x1) in O.block_grid(whole.shape, block):
+        lo = [z0 + (r[0] if z0 > 0 else 0), y0 + (r[1] if y0 > 0 else 0), x0 + (r[2] if x0 > 0 else 0)]
+        hi = [z1 - (r[0] if z1 < whole.shape[0] else 0), y1 - (r[1] if y1 < whole.shape[1] else 0),
+              x1 - (r[2] if x1 < whole.shape[2] else 0)]
+        exact[lo[0]:hi[0], lo[1]:hi[1], lo[2]:hi[2]] = True
+    assert exact.any() and (~exact).any()
+    assert rel[exact].max() < 1e-12
+    assert rel[~exact].max() == rel.max()
+
+
+def test_blocked_delta_psf_needs_no_halo():
+    """L851: with delta PSFs nothing is read from a neighbour: halo 0, any block shape == whole."""
+    views, _, _ = _dependence_exact_case(3, 3)
+    delta = np.zeros((3, 3, 3))
+    delta[1, 1, 1] = 1.0
+    for variant in ("osem", "efficient"):
+        whole = O.deconvolve(views, [delta] * 3, variant, 2)
+        blk = O.deconvolve_blocked(views, [delta] * 3, (7, 5, 11), variant, 2, halo_zyx=(0, 0, 0))
+        assert np.abs(blk - whole).max() / whole.max() < 1e-13      # FFT sizes differ per block: rounding only
+
+
+def test_view_update_is_the_osem_step():
+    """Oracle.view_update(v) (what bench.py times) is exactly one line of eq. 109-112: V of them = iterate(1)."""
+    views, psfs, _ = _dependence_exact_case(3, 4)
+    a = O.Oracle(views, psfs, "osem")
+    b = O.Oracle(views, psfs, "osem")
+    a.iterate(1)
+    for v in range(3):
+        b.view_update(v)
+    assert np.array_equal(a.psi, b.psi) and a.flux == b.flux and a.l1_change == b.l1_change
+    with pytest.raises(ValueError):
+        O.Oracle(views, psfs, "efficient").view_update(0)
+
+
 # --------------------------------------------------------------------------------------
 # section 12 (L891-903): weights of partially overlapping views
 # --------------------------------------------------------------------------------------
