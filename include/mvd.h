@@ -59,7 +59,8 @@ typedef enum {
   MVD_ERR_UNSUPPORTED = 2,   /* no FFT length available for this size */
   MVD_ERR_WORKSPACE = 3,     /* workspace NULL, misaligned or too small */
   MVD_ERR_CUDA = 4,          /* a CUDA call failed (see mvd_last_error) */
-  MVD_ERR_STATE = 5          /* context unusable after an earlier CUDA error */
+  MVD_ERR_STATE = 5          /* call not valid in this state: context broken by an earlier CUDA error, or a
+                              * view-parallel context driven through the wrong calls (see mvd_last_error) */
 } mvd_status;
 
 typedef enum {
@@ -173,7 +174,8 @@ MVD_API mvd_status mvd_get_back_projector(mvd_ctx* ctx, int view, double* dst_ho
 /* One zero-extended "same" convolution of a device volume with view v's PSF (which = 0) or
  * back-projector (which = 1) through the library's FFT path: dst = crop(src (*) kernel).
  * src and dst are DEVICE pointers to N voxels (may alias).  Uses the context's work buffers: the
- * next mvd_iterate re-derives its transform state.  For per-stage parity tests. */
+ * next mvd_iterate re-derives its transform state.  For per-stage parity tests.  In a view-parallel
+ * context only the views it owns have spectra: MVD_ERR_INVALID_ARG for the others. */
 MVD_API mvd_status mvd_convolve(mvd_ctx* ctx, int view, int which, const float* src, float* dst);
 
 /* Number of kernel launches the library has issued on this context since creation. */
@@ -202,7 +204,8 @@ MVD_API const char* mvd_kernel_class_name(int kernel_class);
  * every block by `halo` voxels of neighbouring data per side (clipped at the volume faces; halo
  * = NULL -> PSF half-size), runs `iterations` iterations on each extended block with
  * psi0 = mean over the whole volume, and pastes the central block into dst (DEVICE, N voxels).
- * All device memory comes from opt->workspace (size: mvd_blocked_workspace_size). */
+ * All device memory comes from opt->workspace (size: mvd_blocked_workspace_size).  The whole-volume
+ * options weights, views_ready, local_views, psi0 and psi0_value are refused (MVD_ERR_UNSUPPORTED). */
 MVD_API size_t mvd_blocked_workspace_size(int n_views, const int dims[3], const int (*psf_dims)[3],
                                   mvd_variant variant, const mvd_options* opt,
                                   const int block_dims[3], const int halo[3]);

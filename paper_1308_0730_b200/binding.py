@@ -255,6 +255,8 @@ class Deconvolver:
         self.workspace_bytes = int(nbytes)
         view_ptrs = (C.c_void_p * len(full))(*[None if v is None else v.data_ptr() for v in self.views])
         ctx = C.c_void_p()
+        # the conversions / copies above ran on torch's current stream: the library's stream waits for them
+        self.stream.wait_stream(torch.cuda.current_stream(self.device))
         with torch.cuda.device(self.device):
             st = lib.mvd_create(C.byref(ctx), len(full), view_ptrs, _Int3(*self.dims), psf_ptrs,
                                 C.cast(psf_dims, C.c_void_p), VARIANTS[variant], C.byref(opt))
@@ -397,6 +399,7 @@ def deconvolve_blocked(views, psfs, block_dims, iterations, variant="osem", kern
     opt.stream = stream.cuda_stream
     view_ptrs = (C.c_void_p * len(views))(*[v.data_ptr() for v in views])
     launches = C.c_longlong(0)
+    stream.wait_stream(torch.cuda.current_stream(device))
     with torch.cuda.device(device):
         st = lib.mvd_deconvolve_blocked(len(views), view_ptrs, _Int3(*dims), psf_ptrs,
                                         C.cast(psf_dims, C.c_void_p), VARIANTS[variant], C.byref(opt),
@@ -414,8 +417,11 @@ def reduce_sum(t, stream=None):
     lib = load_library()
     t = t.contiguous()
     stream = stream if stream is not None else torch.cuda.current_stream(t.device)
+    with torch.cuda.device(t.device):
+        nscratch = int(lib.mvd_reduce_scratch_bytes())
     with torch.cuda.stream(stream):
-        scratch = torch.empty(int(lib.mvd_reduce_scratch_bytes()), dtype=torch.uint8, device=t.device)
+        scratch = torch.empty(nscratch, dtype=torch.uint8, device=t.device)
+    stream.wait_stream(torch.cuda.current_stream(t.device))      # t may have been produced on the current stream
     out = C.c_double(0.0)
     with torch.cuda.device(t.device):
         _check(lib.mvd_reduce_sum(t.data_ptr(), t.numel(), scratch.data_ptr(), stream.cuda_stream, C.byref(out)),

@@ -3,12 +3,14 @@
     python -m paper_1308_0730_b200.build [-j N] [--force]
 
 One object per supported pencil length (csrc/lengths.def x csrc/inst.cu) plus csrc/mvd.cu, compiled
-in parallel, cached by modification time under csrc/build/, linked into
+in parallel, cached by modification time under csrc/build/<hash of the compiler flags>/ (so objects of an
+experiment build are never linked into a normal one), linked into
 paper_1308_0730_b200/libmvd.so.  Nothing here runs at import time of the package.
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import os
 import re
 import subprocess
@@ -52,7 +54,12 @@ def _run(cmd):
 
 
 def build(jobs=None, force=False, verbose=True):
+    global OBJ
+    tag = hashlib.sha1(" ".join([NVCC] + FLAGS).encode()).hexdigest()[:10]
+    OBJ = os.path.join(CSRC, "build", tag)
     os.makedirs(OBJ, exist_ok=True)
+    stamp = os.path.join(CSRC, "build", "linked_flags")
+    relink = not os.path.exists(stamp) or open(stamp).read() != tag
     hdr = [os.path.join(CSRC, f) for f in ("fft_reg.cuh", "pass_kernels.cuh", "pass_tma.cuh", "async_copy.cuh", "fft_ops.h")]
     tasks = []
     objs = []
@@ -75,8 +82,9 @@ def build(jobs=None, force=False, verbose=True):
         print("[mvd build] %d objects to compile, %d jobs" % (len(tasks), jobs), flush=True)
     with ThreadPoolExecutor(max_workers=jobs) as ex:
         list(ex.map(_run, tasks))
-    if tasks or not os.path.exists(LIB):
+    if tasks or relink or not os.path.exists(LIB):
         _run([NVCC, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a", "-lcudart"])
+        open(stamp, "w").write(tag)
     if verbose:
         print("[mvd build] %s" % LIB, flush=True)
     return LIB

@@ -149,12 +149,6 @@ MVD_DEV float2 cmul_conj(float2 a, float2 b) {   // a * conj(b) = (a.x b.x + a.y
   const float2 t = mul2(a.y, a.y, b.y, b.x);
   return make_float2(MVD_FMA(a.x, b.x, t.x), MVD_FMA(-a.x, b.y, t.y));
 }
-// a * w for a table entry e = (w.x, w.y, -w.y, w.x): two packed instructions, no sign flip
-MVD_DEV float2 cmul_tab(float2 a, float4 e) {
-  const float2 t = mul2(a.x, a.x, e.x, e.y);
-  return fma2(a.y, a.y, e.z, e.w, t.x, t.y);
-}
-
 // multiply by exp(DIR * 2*pi*i * K / N), K and N compile-time (DIR = -1 forward, +1 inverse)
 template <int K, int N, int DIR>
 MVD_DEV float2 cmul_root(float2 a) {

@@ -138,6 +138,18 @@ static int best_exch_stride(int A, int B, int R, int nthreads, int min_stride, b
   return best;
 }
 
+// SMs of the current device (148 on B200); 148 when there is no device (host-only planning calls)
+static int sm_count() {
+  int dev = 0, n = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+    cudaGetLastError();
+    n = 148;
+  }
+  return n;
+}
+// grid of the grid-stride reduction / fill kernels: 8 CTAs of 256 threads per SM
+static int reduce_blocks() { return 8 * sm_count(); }
+
 static int env_int(const char* name, int dflt) {
   const char* s = getenv(name);
   return (s && *s) ? atoi(s) : dflt;
@@ -322,7 +334,7 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
   P.off_kern = take(P.psf_stride * sizeof(double) * P.V);
   P.off_auto = take(kmode == MVD_KERNEL_COMPOUND ? P.auto_stride * sizeof(double) * P.V : 256);
   P.off_stage = take(P.psf_stride * sizeof(float));
-  P.sum_blocks = 1184;   // 148 SMs x 8
+  P.sum_blocks = reduce_blocks();
   P.off_partials = take(sizeof(double) * 2 * (size_t)std::max(P.nctax, P.sum_blocks));
   P.off_scalars = take(sizeof(double) * (size_t)(P.V + 8));
   P.off_cmp = take(sizeof(double) * (6 * 192 + 8));   // mvd_compare partials
@@ -358,6 +370,7 @@ struct mvd_ctx {
   int use_graph = 0;
   cudaGraphExec_t graph_exec = nullptr;
   long long graph_launches = 0;
+  int graph_stats_ncta = 0;          // CTAs of the update kernel that write the statistics partials (as captured)
   char err[512] = {0};
   int num_sms = 148;
   int xt_blocks[5] = {0, 0, 0, 0, 0};   // resident CTAs per SM of the TMA-staged x pass, per mode
@@ -797,7 +810,7 @@ mvd_status init_estimate(mvd_ctx* c, const float* psi0) {
   if (psi0) {
     MVD_CK(cudaMemcpyAsync(c->psi(), psi0, sizeof(float) * P.nvox, cudaMemcpyDeviceToDevice, c->stream), "psi0 copy");
   } else if (c->psi0_value > 0.f) {
-    fill_value_kernel<<<1184, 256, 0, c->stream>>>(c->psi(), P.nvox, c->psi0_value);
+    fill_value_kernel<<<P.sum_blocks, 256, 0, c->stream>>>(c->psi(), P.nvox, c->psi0_value);
     MVD_CK(cudaGetLastError(), "fill_value_kernel");
     ++c->launches;
   } else if (c->partial) {
@@ -812,7 +825,7 @@ mvd_status init_estimate(mvd_ctx* c, const float* psi0) {
       MVD_CK(cudaGetLastError(), "final_sum_kernel");
       c->launches += 2;
     }
-    fill_mean_kernel<<<1184, 256, 0, c->stream>>>(c->psi(), P.nvox, c->scalars(), P.V, (double)P.nvox * P.V);
+    fill_mean_kernel<<<P.sum_blocks, 256, 0, c->stream>>>(c->psi(), P.nvox, c->scalars(), P.V, (double)P.nvox * P.V);
     MVD_CK(cudaGetLastError(), "fill_mean_kernel");
     ++c->launches;
   }
@@ -962,7 +975,11 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
 
 mvd_status mvd_iterate(mvd_ctx* c, int n) {
   if (!c || n < 0) return MVD_ERR_INVALID_ARG;
-  if (c->broken || c->partial) return MVD_ERR_STATE;   // view-parallel contexts: mvd_partial_product / mvd_apply_product
+  if (c->broken) return MVD_ERR_STATE;
+  if (c->partial) {   // view-parallel contexts advance through mvd_partial_product / mvd_apply_product
+    snprintf(c->err, sizeof(c->err), "view-parallel context: use mvd_partial_product / mvd_apply_product");
+    return MVD_ERR_STATE;
+  }
   if (n == 0) return MVD_OK;
   MVD_TRY(ensure_w(c));
   if (c->use_graph) {
@@ -972,18 +989,26 @@ mvd_status mvd_iterate(mvd_ctx* c, int n) {
       MVD_CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal), "graph capture begin");
       mvd_status s = iteration_body(c);
       cudaError_t e = cudaStreamEndCapture(c->stream, &g);
-      if (s != MVD_OK) return s;
+      if (s != MVD_OK || e != cudaSuccess) {
+        if (g) cudaGraphDestroy(g);
+        if (s != MVD_OK) return s;
+      }
       MVD_CK(e, "graph capture end");
       c->graph_launches = c->launches - before;
       c->launches = before;
-      MVD_CK(cudaGraphInstantiate(&c->graph_exec, g, 0), "graph instantiate");
+      c->graph_stats_ncta = c->stats_ncta;
+      e = cudaGraphInstantiate(&c->graph_exec, g, 0);
       cudaGraphDestroy(g);
+      MVD_CK(e, "graph instantiate");
     }
     for (int i = 0; i < n; ++i) {
       MVD_CK(cudaGraphLaunch(c->graph_exec, c->stream), "graph launch");
       c->launches += c->graph_launches;
       ++c->iters;
     }
+    // the replayed update kernel wrote its partials: same statistics as the plain launches
+    c->stats_valid = true;
+    c->stats_ncta = c->graph_stats_ncta;
     return MVD_OK;
   }
   for (int i = 0; i < n; ++i) {
@@ -1064,16 +1089,18 @@ mvd_status mvd_apply_product(mvd_ctx* c, int total_views) {
   return MVD_OK;
 }
 
-size_t mvd_reduce_scratch_bytes(void) { return sizeof(double) * (1184 + 8); }
+size_t mvd_reduce_scratch_bytes(void) { return sizeof(double) * (size_t)(mvd::reduce_blocks() + 8); }
 
 mvd_status mvd_reduce_sum(const float* src, long long n, void* scratch, void* stream, double* host_out) {
   if (!src || n < 0 || !scratch || !host_out) return MVD_ERR_INVALID_ARG;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   double* part = reinterpret_cast<double*>(scratch);
-  sum_f32_kernel<<<1184, 256, 0, st>>>(src, n, part);
-  final_sum_kernel<<<1, 256, 0, st>>>(part, 1184, 1, part + 1184);
+  const int nb = mvd::reduce_blocks();
+  sum_f32_kernel<<<nb, 256, 0, st>>>(src, n, part);
   if (cudaGetLastError() != cudaSuccess) return MVD_ERR_CUDA;
-  if (cudaMemcpyAsync(host_out, part + 1184, sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+  final_sum_kernel<<<1, 256, 0, st>>>(part, nb, 1, part + nb);
+  if (cudaGetLastError() != cudaSuccess) return MVD_ERR_CUDA;
+  if (cudaMemcpyAsync(host_out, part + nb, sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
       cudaStreamSynchronize(st) != cudaSuccess)
     return MVD_ERR_CUDA;
   return MVD_OK;
@@ -1139,6 +1166,10 @@ mvd_status mvd_get_back_projector(mvd_ctx* c, int view, double* dst_host) {
 mvd_status mvd_convolve(mvd_ctx* c, int view, int which, const float* src, float* dst) {
   if (!c || !src || !dst || view < 0 || view >= c->P.V || which < 0 || which > 1) return MVD_ERR_INVALID_ARG;
   if (c->broken) return MVD_ERR_STATE;
+  if (!c->is_local[view]) {   // view-parallel context: no spectra were built for views of other ranks
+    snprintf(c->err, sizeof(c->err), "view %d belongs to another rank of this view-parallel context", view);
+    return MVD_ERR_INVALID_ARG;
+  }
   c->w_valid = false;
   MVD_TRY(x_load(c, src, c->W()));
   MVD_TRY(conv_core(c, nullptr, c->W(), which ? c->specK(view) : c->specH(view), false));
@@ -1192,7 +1223,7 @@ const char* mvd_status_string(mvd_status s) {
     case MVD_ERR_UNSUPPORTED: return "unsupported size (no FFT length available)";
     case MVD_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
     case MVD_ERR_CUDA: return "CUDA error";
-    case MVD_ERR_STATE: return "context unusable after an earlier CUDA error";
+    case MVD_ERR_STATE: return "call not valid in this state of the context (see mvd_last_error)";
   }
   return "unknown status";
 }
@@ -1254,7 +1285,7 @@ mvd_status blocked_layout(BlockedLayout& L, int n_views, const int dims[3], cons
   }
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t at = off; off = align_up(off + bytes, 256); return at; };
-  L.off_scal = take(sizeof(double) * (size_t)(1184 + n_views + 8));
+  L.off_scal = take(sizeof(double) * (size_t)(reduce_blocks() + n_views + 8));
   L.off_views = take(align_up(L.max_ext * sizeof(float), 256) * n_views);
   L.off_psi0 = take(L.max_ext * sizeof(float));
   L.off_est = take(L.max_ext * sizeof(float));
@@ -1289,7 +1320,8 @@ extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* vi
   if (!views || !psfs || !dst || !opt_in || iterations < 0) return MVD_ERR_INVALID_ARG;
   mvd_options tmp;
   const mvd_options* opt = defaults(opt_in, &tmp);
-  if (opt->weights || opt->views_ready) return MVD_ERR_UNSUPPORTED;   // whole-volume options
+  if (opt->weights || opt->views_ready || opt->local_views || opt->psi0 || opt->psi0_value != 0.f)
+    return MVD_ERR_UNSUPPORTED;   // whole-volume options
   BlockedLayout L;
   mvd_status s = blocked_layout(L, n_views, dims, psf_dims, variant, opt, block_dims, halo);
   if (s != MVD_OK) return s;
@@ -1298,7 +1330,8 @@ extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* vi
   char* ws = reinterpret_cast<char*>(opt->workspace);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(opt->stream);
   double* partial = reinterpret_cast<double*>(ws + L.off_scal);
-  double* sums = partial + 1184;
+  const int nb = reduce_blocks();
+  double* sums = partial + nb;
   const size_t vstride = align_up(L.max_ext * sizeof(float), 256);
   std::vector<const float*> bviews(n_views);
   for (int v = 0; v < n_views; ++v) bviews[v] = reinterpret_cast<const float*>(ws + L.off_views + v * vstride);
@@ -1311,11 +1344,11 @@ extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* vi
   // psi^0 = mean over the WHOLE volume and all views (R13), kept on the device
   for (int v = 0; v < n_views; ++v) {
     if (!views[v]) return MVD_ERR_INVALID_ARG;
-    sum_f32_kernel<<<1184, 256, 0, st>>>(views[v], nvox, partial);
-    final_sum_kernel<<<1, 256, 0, st>>>(partial, 1184, 1, sums + v);
+    sum_f32_kernel<<<nb, 256, 0, st>>>(views[v], nvox, partial);
+    final_sum_kernel<<<1, 256, 0, st>>>(partial, nb, 1, sums + v);
     launches += 2;
   }
-  fill_mean_kernel<<<1184, 256, 0, st>>>(psi0, (long long)L.max_ext, sums, n_views, (double)nvox * n_views);
+  fill_mean_kernel<<<nb, 256, 0, st>>>(psi0, (long long)L.max_ext, sums, n_views, (double)nvox * n_views);
   ++launches;
   if (cudaGetLastError() != cudaSuccess) return MVD_ERR_CUDA;
 
@@ -1341,7 +1374,7 @@ extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* vi
     }
     const Dims3 E{d[0], d[1], d[2]};
     const long long ext = (long long)d[0] * d[1] * d[2];
-    const unsigned grid = (unsigned)std::min<long long>((ext + 255) / 256, 1184 * 8);
+    const unsigned grid = (unsigned)std::min<long long>((ext + 255) / 256, (long long)nb * 8);
     for (const Seg& sz : L.seg[2])
       for (const Seg& sy : L.seg[1])
         for (const Seg& sx : L.seg[0]) {

@@ -38,17 +38,6 @@ struct PassCfg {
 
 MVD_DEV float2 ld_tw(const float2* tw, int idx) { return __ldg(tw + idx); }
 
-// pw[k] = w^k, balanced products (depth <= log2 k)
-template <int N>
-MVD_DEV void powers(float2 w, float2 (&pw)[N]) {
-  pw[0] = make_float2(1.f, 0.f);
-  if constexpr (N > 1) pw[1] = w;
-  static_for<2, N>([&](auto k_) {
-    constexpr int k = decltype(k_)::value;
-    pw[k] = cmul(pw[k / 2], pw[k - k / 2]);
-  });
-}
-
 // =========================================================================================
 // strided pencil FFT, form F, direction DIR (-1 forward, +1 inverse; unnormalised)
 // =========================================================================================

@@ -376,6 +376,8 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
         });
       }
     }
+    // the tile was transformed in place by ordinary stores; the copy engine (async proxy) refills it
+    fence_proxy_async();
     __syncthreads();   // every read of this tile is done
     if (tid == 0 && more && nst == 1) issue(tile + (int)gridDim.x, 0);   // one stage: refill it now
   }
@@ -511,6 +513,7 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
         });
       }
     }
+    fence_proxy_async();   // in-place stores to the tile before the copy engine refills it
     __syncthreads();
     if (tid == 0 && more && nst == 1) issue_in(tile + (int)gridDim.x, 0);   // one input stage: refill now
   }

@@ -250,6 +250,33 @@ def test_set_estimate_resume_and_graph_replay(mvd, tiny):
         mvd.Deconvolver(to_dev(tiny.views), tiny.psfs, use_graph=True, stream=torch.cuda.default_stream())
 
 
+@pytest.mark.parametrize("variant", ["osem", "efficient"])
+def test_stats_after_set_estimate_graph_equals_plain_and_oracle(mvd, tiny, variant):
+    """mvd_get_stats after mvd_set_estimate + mvd_iterate: the replayed graph's update kernel wrote its
+    partials, so graph and plain-launch contexts report the same flux and l1_change, those of the oracle."""
+    import torch
+    start = (tiny.gt * 0.5 + 7.0).astype(np.float32)
+    o = O.Oracle(tiny.views, tiny.psfs, variant, psi0=start)
+    o.iterate(2)
+    got = {}
+    for use_graph in (False, True):
+        torch.cuda.synchronize()
+        kw = {"use_graph": True, "stream": torch.cuda.Stream()} if use_graph else {}
+        d = mvd.Deconvolver(to_dev(tiny.views), tiny.psfs, variant=variant, **kw)
+        d.iterate(1)                                     # the graph is captured on some other estimate
+        d.set_estimate(torch.from_numpy(start).cuda())
+        st0 = d.get_stats()                              # no update since set_estimate: flux of psi, no change
+        assert st0["l1_change"] == 0.0 and st0["flux"] == pytest.approx(float(start.astype(np.float64).sum()), rel=1e-6)
+        d.iterate(2)
+        got[use_graph] = (d.get_stats(), d.get_estimate_host())
+        d.close()
+    assert got[True][0]["flux"] == got[False][0]["flux"] and got[True][0]["l1_change"] == got[False][0]["l1_change"]
+    assert np.array_equal(got[True][1], got[False][1])
+    assert got[True][0]["l1_change"] > 0
+    assert got[True][0]["flux"] == pytest.approx(o.flux, rel=1e-5)
+    assert got[True][0]["l1_change"] == pytest.approx(o.l1_change, rel=2e-3)
+
+
 def test_eps_and_floor_clamps(mvd, tiny):
     """R4: zero-valued data drive psi to the floor on both sides identically."""
     views = [v.copy() for v in tiny.views]
@@ -320,16 +347,52 @@ def test_blocked_single_block_equals_whole(mvd, tiny):
 # ------------------------------------------------------------------------------------------
 # BASELINE config 4 at full size, in the launch configuration bench.py times (CUDA graph replay)
 # ------------------------------------------------------------------------------------------
-def test_config4_bench_configuration(mvd):
+@pytest.fixture(scope="module")
+def config4():
+    return mvd_synth.make_problem(4)
+
+
+def test_config4_bench_configuration(mvd, config4):
     """512x512x256, 7 views, efficient-OSEM, one CUDA graph per iteration: every voxel against the
-    oracle after 1 and 2 iterations (14 view-updates; the oracle needs ~15 s per iteration)."""
-    p = mvd_synth.make_problem(4)
-    g, st = gpu_checkpoints(mvd, p, "osem", "auto", (1, 2), use_graph=True)
-    o, orc = oracle_checkpoints(p, "osem", "auto", (1, 2))
+    oracle after 1, 2 and 10 iterations (north_star: rel-L2 <= 1e-5 after 1 iteration, <= 1e-4 after 10,
+    max per-voxel rel <= 1e-3).  70 view-updates; the oracle needs ~13 s per iteration on 16 cores."""
+    p = config4
+    g, st = gpu_checkpoints(mvd, p, "osem", "auto", (1, 2, 10), use_graph=True)
+    o, orc = oracle_checkpoints(p, "osem", "auto", (1, 2, 10))
     check(g[1], o[1], 1, "config 4")
     l2, mx = errors(g[2], o[2])
     assert l2 <= 2e-5 and mx <= TOL_MAX, (l2, mx)      # 2 iterations: well inside the 10-iteration bound
+    check(g[10], o[10], 10, "config 4")
+    assert st["iterations_done"] == 10
     assert st["flux"] == pytest.approx(orc.flux, rel=1e-5)
+    assert st["l1_change"] == pytest.approx(orc.l1_change, rel=2e-3)
+
+
+def _combined_variants_plain_and_graph(mvd, p, what):
+    """independent (eq. 70) and efficient (eq. 104) with the root of eq. 44: the shared forward pass
+    (W0), the product accumulation and the powf root of the X_ACCUM kernels, as plain launches and
+    under CUDA-graph replay, against the oracle after 1 and 3 iterations."""
+    for variant in ("independent", "efficient"):
+        o, orc = oracle_checkpoints(p, variant, "auto", (1, 3))
+        plain, st = gpu_checkpoints(mvd, p, variant, "auto", (1, 3))
+        graph, stg = gpu_checkpoints(mvd, p, variant, "auto", (1, 3), use_graph=True)
+        for c in (1, 3):
+            check(plain[c], o[c], c, "%s %s" % (what, variant))
+            assert np.array_equal(plain[c], graph[c]), (what, variant, c)
+        assert st["flux"] == pytest.approx(orc.flux, rel=1e-5)
+        assert stg == st                                 # graph replay reports the same statistics
+
+
+def test_config3_combined_variants(mvd):
+    _combined_variants_plain_and_graph(mvd, mvd_synth.make_problem(3), "config 3")
+
+
+def test_config4_combined_variants(mvd, config4):
+    _combined_variants_plain_and_graph(mvd, config4, "config 4")
+
+
+def test_config1_combined_variants(mvd):
+    _combined_variants_plain_and_graph(mvd, mvd_synth.make_problem(1), "config 1")
 
 
 # ------------------------------------------------------------------------------------------
