@@ -17,8 +17,17 @@ bytes / live CUDA-event time), `kernels` (every class), `cpu_baseline` (the fp64
 this box's host cores on a bounded sample), `e2e` (whole job through the public API from pinned
 host buffers: H2D of the views, mvd_create, all iterations, D2H of the estimate).
 
---impl reference times the oracle itself (rank 0 only), one view-update of the same recipe at
-256x256x128 per step.
+`sustained`: the same step replayed back to back for >= 3 s (the board reaches its power cap), with its
+own clock summary.  --impl reference times the oracle itself (rank 0 only): one view-update of
+efficient-OSEM per step on the SAME workload (config 4 at full size: about 2 s per step on 16 cores).
+
+Other workloads, each still one JSON line:
+    --config 5                    BASELINE configs[4] whole (1024x1024x512, 6 views)
+    --config 5 --blocked 256      the same volume as 256^3 blocks + halo r (mvd_deconvolve_blocked, 5 iterations)
+    --config 5 --psf-sweep        one record per PSF box 9^3 ... 31x31x63 in "sweep"
+    --mode view-parallel          combined efficient variant, views dealt over the ranks, one all-reduce(PRODUCT)
+                                  per iteration; scaling "strong"
+    --mode block-replicas         config 5 blocks dealt over the ranks (the paper's 2-GPU mode, L225); "strong"
 """
 from __future__ import annotations
 
@@ -149,16 +158,23 @@ def hbm_peak():
 
 
 def ncu_traffic(kernel_class, k):
-    """dram bytes per launch of the class from the committed ncu --set full capture, or None."""
-    p = os.path.join(ROOT, "profiles", "r01f_traffic.csv")
-    try:
-        for line in open(p).read().splitlines()[1:]:
-            cfg, cls, val = line.split(",")
-            if int(cfg) == k and cls == kernel_class:
-                return int(val)
-    except Exception:
-        pass
-    return None
+    """(dram bytes per launch of the class, source string) from the newest committed `ncu --set full`
+    capture (profiles/r*_traffic.csv; its first line is a comment naming the commit it was taken at),
+    or (None, None)."""
+    import glob
+    for p in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.csv")), reverse=True):
+        try:
+            lines = open(p).read().splitlines()
+            stamp = lines[0].lstrip("# ").strip() if lines and lines[0].startswith("#") else "build not recorded"
+            for line in lines:
+                if line.startswith("#") or line.startswith("config"):
+                    continue
+                cfg, cls, val = line.split(",")
+                if int(cfg) == k and cls == kernel_class:
+                    return int(val), "%s (%s)" % (os.path.relpath(p, ROOT), stamp)
+        except Exception:
+            continue
+    return None, None
 
 
 # ------------------------------------------------------------------------------------------
@@ -210,7 +226,7 @@ def cpu_baseline(prob, budget_s=12.0):
     n = 0
     t0 = time.perf_counter()
     while n < prob.n_views:
-        o._commit(np.maximum(o.psi * o.factor(n), o.psi_floor))   # one step of Oracle.iterate's OSEM loop
+        o.view_update(n)                                          # one line of eq. 109-112, as Oracle.iterate runs it
         n += 1
         if time.perf_counter() - t0 > budget_s:
             break
@@ -219,6 +235,31 @@ def cpu_baseline(prob, budget_s=12.0):
     return {"value": nvox * n / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": "first %d of %d view-updates of one efficient-OSEM iteration on the full %dx%dx%d volume "
                       "(fp64, scipy.fft with %d workers), %.1f s" % (n, prob.n_views, *prob.dims, cores, dt)}
+
+
+SWEEP_BOXES = ((9, 9, 9), (13, 13, 27), (17, 17, 35), (21, 21, 45), (25, 25, 51), (31, 31, 63))   # BASELINE configs[4]
+
+
+def sweep_psfs(k, box):
+    """PSFs of config k's recipe on another box: sigma_xy = r_x / 4, sigma_z = r_z / 3.5."""
+    import mvd_synth
+    rec = mvd_synth.CONFIGS[k]
+    sxy, sz = max((box[0] - 1) / 2 / 4.0, 0.5), max((box[2] - 1) / 2 / 3.5, 0.5)
+    return [mvd_synth.gaussian_psf(box, sxy, sz, a) for a in rec["angles"]]
+
+
+def time_steps(d, stream, steps, barrier):
+    """CUDA-event time (ms) of `steps` calls of d.iterate(1) on the library's stream, plus the wall-clock window."""
+    import torch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.perf_counter()
+    e0.record(stream)
+    for _ in range(steps):
+        d.iterate(1)
+    e1.record(stream)
+    barrier()
+    return e0.elapsed_time(e1), t0, time.perf_counter()
 
 
 def run_ours(args):
@@ -243,18 +284,136 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     k = args.config
+    if args.mode == "block-replicas" or args.blocked or args.psf_sweep:
+        k = args.config = 5 if args.config == 4 else args.config      # these are config-5 workloads (BASELINE configs[4])
     t = time.perf_counter()
     prob = load_problem(k, rank, world, dist)
     log("[bench] rank %d: config %d drawn in %.1f s" % (rank, k, time.perf_counter() - t))
     V, dims = prob.n_views, prob.dims
     nvox = float(np.prod(dims))
 
-    host_views = [torch.from_numpy(v).pin_memory() for v in prob.views]
+    host_views = [torch.from_numpy(v).pin_memory() for v in prob.views] if not (args.blocked or args.psf_sweep or args.mode != "replicas") \
+        else [torch.from_numpy(v) for v in prob.views]
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
         dev_views = [h.to("cuda", non_blocking=True) for h in host_views]
     stream.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    peak, peak_src = hbm_peak()
+    base = {"metric": METRIC, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "higher_is_better": True, "vs_baseline": None, "dtype": "f32", "data": "synthetic"}
+    wl = "BASELINE configs[%d]: %dx%dx%d, %d views, PSF %dx%dx%d" % (k - 1, *dims, V, *prob.psf_dims)
 
+    def emit(line):
+        sampler.stop()
+        if rank == 0:
+            print(json.dumps(line), flush=True)
+        if world > 1:
+            dist.destroy_process_group()
+
+    # ============================ view-parallel combined variant ============================
+    if args.mode == "view-parallel":
+        # eq. 104 + eq. 44 with the views dealt round-robin over the ranks: per iteration each
+        # rank's partial product, ONE all-reduce(PRODUCT) of N floats over NCCL, the same root update everywhere
+        if V < world:
+            raise SystemExit("bench.py: view-parallel needs at least one view per rank (%d views, %d ranks)" % (V, world))
+        mine = mvd.split_views(V, world, rank)
+        d = mvd.ViewParallelDeconvolver([dev_views[v] for v in mine], prob.psfs, variant="efficient", rank=rank,
+                                        world=world, group=None, stream=stream)
+        for v in range(V):
+            if v not in mine:
+                dev_views[v] = None
+        torch.cuda.empty_cache()
+        for _ in range(args.warmup):
+            d.iterate(1)
+        launches0 = d.d.launch_count
+        ms, t0, t1 = time_steps(d, stream, args.steps, barrier)
+        launches = d.d.launch_count - launches0
+        ms = max_over_ranks([ms], world, dist, "cuda")[0]
+        stats = d.get_stats()
+        if not np.isfinite(stats["flux"]):
+            raise SystemExit("bench.py: non-finite estimate")
+        line = dict(base, value=nvox * V * args.steps / (ms * 1e-3) / 1e9, ms_per_step=ms / args.steps, scaling="strong",
+                    config={"workload": wl + ", combined efficient variant (MVD_EFFICIENT), one step = one iteration",
+                            "fft_dims": list(d.d.fft_dims), "voxel_views_per_step": nvox * V,
+                            "parallelism": "view-parallel x%d: views %s on rank 0; one all-reduce(PRODUCT) of %.0f MB per "
+                                           "iteration" % (world, mine, nvox * 4 / 1e6),
+                            "l2": "inputs larger than L2", "cuda_graph": False},
+                    clocks=sampler.summary(t0, t1), gpu_launches=launches, e2e=None, roofline=None, flux=stats["flux"])
+        d.close()
+        return emit(line)
+
+    # ============================ block-wise processing (config 5) ============================
+    if args.blocked or args.mode == "block-replicas":
+        # R13 / PAPER.md L943, L225: 256^3 blocks + halo r, every block an independent problem; with several ranks
+        # the blocks are dealt round-robin (the paper's two-GPU mode) and no rank talks to another
+        B = args.blocked or 256
+        iters = prob.iterations
+        kw = dict(block_rank=rank, block_world=world) if args.mode == "block-replicas" else {}
+        reps = []
+        for rep in range(1 + max(1, args.repeats)):                    # first pass = warm-up (allocator, attributes)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            barrier()
+            t0 = time.perf_counter()
+            e0.record(stream)
+            out, launches = mvd.deconvolve_blocked(dev_views, prob.psfs, (B, B, B), iters, variant="osem", stream=stream, **kw)
+            e1.record(stream)
+            barrier()
+            t1 = time.perf_counter()
+            if rep:
+                reps.append(e0.elapsed_time(e1))
+            if not bool(torch.isfinite(out[::37, ::41, ::43]).all()):
+                raise SystemExit("bench.py: non-finite estimate")
+            del out
+        ms = max_over_ranks([float(np.median(reps))], world, dist, "cuda")[0]
+        nblocks = int(np.prod([-(-n // B) for n in dims]))
+        replicas = args.mode != "block-replicas"
+        units = nvox * V * iters * (world if replicas else 1)
+        line = dict(base, steps=iters, warmup=1, value=units / (ms * 1e-3) / 1e9, ms_per_step=ms / iters,
+                    scaling="weak" if replicas else "strong",
+                    config={"workload": wl + ", efficient-OSEM as %d blocks of %d^3 + halo r (mvd_deconvolve_blocked: gather, "
+                                             "per-shape contexts and precompute, %d iterations per block, paste); value counts "
+                                             "the useful (un-padded, un-haloed) voxels" % (nblocks, B, iters),
+                            "parallelism": ("replicas x%d" % world) if replicas else "blocks dealt round-robin over %d ranks, no collective" % world,
+                            "l2": "inputs larger than L2", "cuda_graph": False, "ms_total": ms, "repeats": len(reps)},
+                    clocks=sampler.summary(t0, t1), gpu_launches=launches, e2e=None, roofline=None)
+        return emit(line)
+
+    # ============================ PSF-size sweep (config 5, whole volume) ============================
+    if args.psf_sweep:
+        # the PSF size drives the padding (and the block overhead).  The views are those of the config-5
+        # draw (timing does not depend on the values); only the PSF box handed to the library changes
+        sweep = []
+        for box in SWEEP_BOXES:
+            psfs = sweep_psfs(k, box)
+            d = mvd.Deconvolver(dev_views, psfs, variant="osem", stream=stream, use_graph=True)
+            for _ in range(args.warmup):
+                d.iterate(1)
+            ms, t0, t1 = time_steps(d, stream, args.steps, barrier)
+            alg = algorithmic_bytes(dims, d.fft_dims)
+            step_bytes = V * (2 * alg["y_fwd"] + 2 * alg["y_inv"] + 2 * alg["z_conv"] + alg["x_quot"] + alg["x_update"])
+            per = ms / args.steps
+            sweep.append({"psf_box": list(box), "fft_dims": list(d.fft_dims), "ms_per_step": per,
+                          "value": nvox * V / (per * 1e-3) / 1e9, "algorithmic_bytes_per_vv": step_bytes / (nvox * V),
+                          "achieved_gbs": step_bytes / (per * 1e-3) / 1e9,
+                          "frac_of_measured": step_bytes / (per * 1e-3) / 1e9 / peak,
+                          "frac_of_nominal_8TBs": step_bytes / (per * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+                          "workspace_gb": d.workspace_bytes / 1e9, "sm_mhz": sampler.summary(t0, t1)["sm_mhz"]})
+            log("[bench] sweep %s: %.2f ms" % (box, per))
+            d.close()
+            del d
+            torch.cuda.empty_cache()
+        ref = [r for r in sweep if tuple(r["psf_box"]) == tuple(prob.psf_dims)] or sweep[-1:]
+        line = dict(base, value=ref[0]["value"], ms_per_step=ref[0]["ms_per_step"], scaling="weak",
+                    config={"workload": wl + " swept over PSF boxes 9^3 ... 31x31x63, efficient-OSEM, whole volume; `value` is the "
+                                             "%dx%dx%d record" % tuple(ref[0]["psf_box"]), "cuda_graph": True,
+                            "l2": "inputs larger than L2", "parallelism": "single GPU"},
+                    clocks=sampler.summary(0, time.perf_counter()), gpu_launches=None, e2e=None, roofline=None, sweep=sweep,
+                    peak_source=peak_src)
+        return emit(line)
+
+    # ============================ the headline workload: replicas of efficient-OSEM ============================
     use_graph = not args.no_graph
     t = time.perf_counter()
     d = mvd.Deconvolver(dev_views, prob.psfs, variant="osem", stream=stream, use_graph=use_graph)
@@ -265,27 +424,24 @@ def run_ours(args):
     # ---- device-resident timing: W warm-up steps, then exactly K steps ---------------------------
     # The timed region replays each iteration as one CUDA graph (the library's use_graph option):
     # the same 8V kernel launches, without the host launch gaps.
-    sampler = ClockSampler(local)
-    sampler.start()
     for _ in range(args.warmup):
         d.iterate(1)
     launches0 = d.launch_count
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    t0 = time.perf_counter()
-    e0.record(stream)
-    for _ in range(args.steps):
-        d.iterate(1)
-    e1.record(stream)
-    barrier()
-    t1 = time.perf_counter()
-    ms = e0.elapsed_time(e1)
+    ms, t0, t1 = time_steps(d, stream, args.steps, barrier)
     launches = d.launch_count - launches0
     clocks = sampler.summary(t0, t1)
-    sampler.stop()
     stats = d.get_stats()
     if not np.isfinite(stats["flux"]):
         raise SystemExit("bench.py: non-finite estimate")
+
+    # ---- sustained: the same step back to back for >= sustained_s seconds (power cap reached) ----
+    sustained = None
+    if args.sustained_s > 0:
+        n = max(args.steps, int(np.ceil(args.sustained_s * 1e3 / (ms / args.steps))))
+        ms_s, s0, s1 = time_steps(d, stream, n, barrier)
+        ms_s = max_over_ranks([ms_s], world, dist, "cuda")[0]
+        sustained = {"steps": n, "seconds": ms_s * 1e-3, "ms_per_step": ms_s / n,
+                     "value": replica_throughput(world, nvox * V, n, ms_s), "unit": UNIT, "clocks": sampler.summary(s0, s1)}
 
     # ---- the same K steps as plain launches with a CUDA-event pair around every launch: the
     #      per-kernel durations behind `kernels` and `roofline` (a graph cannot carry those events) --
@@ -295,13 +451,7 @@ def run_ours(args):
         for _ in range(args.warmup):
             d.iterate(1)
     d.profile(True)
-    barrier()
-    e0.record(stream)
-    for _ in range(args.steps):
-        d.iterate(1)
-    e1.record(stream)
-    barrier()
-    ms_plain = e0.elapsed_time(e1)
+    ms_plain, _, _ = time_steps(d, stream, args.steps, barrier)
     classes = d.profile_read()
     d.profile(False)
 
@@ -309,26 +459,30 @@ def run_ours(args):
     value = replica_throughput(world, nvox * V, args.steps, ms)
 
     # ---- roofline of the dominant kernel class --------------------------------------------------
-    peak, peak_src = hbm_peak()
     alg = algorithmic_bytes(dims, fft_dims)
     kernels = {}
     for name, (tms, n) in classes.items():
         if n:
             per = tms / n
-            kernels[name] = {"launches": n, "avg_ms": per, "share": tms / ms,
+            kernels[name] = {"launches": n, "avg_ms": per, "share": tms / ms_plain,
                              "algorithmic_bytes": alg[name], "achieved_gbs": alg[name] / (per * 1e-3) / 1e9}
     step_bytes = sum(alg[name] * kk["launches"] for name, kk in kernels.items()) / max(args.steps, 1)
     roofline = None
     if kernels:
         top = max(kernels, key=lambda n: kernels[n]["share"])
         a = kernels[top]["achieved_gbs"]
+        traffic, traffic_src = ncu_traffic(top, k)
         roofline = {"bound": "hbm", "kernel": top, "achieved": a, "peak": peak, "unit": "GB/s", "frac": a / peak,
-                    "traffic": ncu_traffic(top, k), "peak_source": peak_src,
+                    "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                     "algorithmic_bytes_per_launch": alg[top],
                     "step": {"algorithmic_bytes": step_bytes,
                              "achieved": step_bytes / (ms / args.steps * 1e-3) / 1e9,
                              "frac_of_measured": step_bytes / (ms / args.steps * 1e-3) / 1e9 / peak,
                              "frac_of_nominal_8TBs": step_bytes / (ms / args.steps * 1e-3) / 1e9 / NOMINAL_HBM_GBS}}
+        if sustained:
+            sustained["achieved_gbs"] = step_bytes / (sustained["ms_per_step"] * 1e-3) / 1e9
+            sustained["frac_of_measured"] = sustained["achieved_gbs"] / peak
+            sustained["frac_of_nominal_8TBs"] = sustained["achieved_gbs"] / NOMINAL_HBM_GBS
 
     # ---- end to end from pinned host buffers, through the public API -----------------------------
     e2e = None
@@ -375,25 +529,16 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_cpu:
         cpu = cpu_baseline(prob)
 
-    if rank == 0:
-        line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "BASELINE configs[%d]: %dx%dx%d, %d views, PSF %dx%dx%d, efficient-OSEM "
-                                   "(MVD_OSEM + compound kernels), one step = one iteration" % (k - 1, *dims, V, *prob.psf_dims),
-                       "fft_dims": list(fft_dims), "voxel_views_per_step": nvox * V,
-                       "parallelism": "replicas x%d (no data-path collective)" % world,
-                       "l2": "inputs larger than L2 (one view-update streams %.1f GB)" % (step_bytes / V / 1e9 if kernels else 0.0),
-                       "cuda_graph": bool(use_graph)},
-            "clocks": clocks, "gpu_launches": launches, "e2e": e2e,
-            "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu,
-            "create_ms": create_ms, "ms_per_step_plain_launches_with_events": ms_plain / args.steps,
-            "workspace_gb": workspace_gb, "flux": stats["flux"],
-        }
-        print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    line = dict(base, value=value, ms_per_step=ms / args.steps, scaling="weak",
+                config={"workload": wl + ", efficient-OSEM (MVD_OSEM + compound kernels), one step = one iteration",
+                        "fft_dims": list(fft_dims), "voxel_views_per_step": nvox * V,
+                        "parallelism": "replicas x%d (no data-path collective)" % world,
+                        "l2": "inputs larger than L2 (one view-update streams %.1f GB)" % (step_bytes / V / 1e9 if kernels else 0.0),
+                        "cuda_graph": bool(use_graph)},
+                clocks=clocks, gpu_launches=launches, e2e=e2e, roofline=roofline, kernels=kernels, sustained=sustained,
+                cpu_baseline=cpu, create_ms=create_ms, ms_per_step_plain_launches_with_events=ms_plain / args.steps,
+                workspace_gb=workspace_gb, flux=stats["flux"])
+    emit(line)
 
 
 # ------------------------------------------------------------------------------------------
@@ -408,33 +553,28 @@ def run_reference(args):
     from oracle import mvd_oracle as O
 
     k = args.config
-    rec = mvd_synth.CONFIGS[k]
-    dims = tuple(max(16, n // 2) for n in rec["dims"]) if k >= 4 else rec["dims"]
-    prob = mvd_synth.make_problem(k, dims=dims)
+    prob = mvd_synth.make_problem(k)                     # the SAME workload as our arm, at full size
+    dims = prob.dims
     cores = len(os.sched_getaffinity(0))
     o = O.Oracle(prob.views, prob.psfs, "osem")
     V = prob.n_views
     nvox = float(np.prod(dims))
 
-    def step(i):
-        v = i % V
-        o._commit(np.maximum(o.psi * o.factor(v), o.psi_floor))
-
     for i in range(args.warmup):
-        step(i)
+        o.view_update(i % V)
     t0 = time.perf_counter()
     for i in range(args.steps):
-        step(args.warmup + i)
+        o.view_update((args.warmup + i) % V)
     dt = time.perf_counter() - t0
     value = nvox * args.steps / dt / 1e9
-    sample = ("one view-update of efficient-OSEM per step (views in index order) on the config-%d recipe at "
-              "%dx%dx%d, %d views, PSF %dx%dx%d; fp64 numpy/scipy.fft, %d workers"
-              % (k, *dims, V, *prob.psf_dims, cores))
+    sample = ("BASELINE configs[%d]: %dx%dx%d, %d views, PSF %dx%dx%d, efficient-OSEM; the oracle as it stands (fp64 "
+              "numpy/scipy.fft, %d workers); each step is ONE view-update (1/%d of an iteration, views in index order) of "
+              "the full volume" % (k - 1, *dims, V, *prob.psf_dims, cores, V))
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": sample},
+        "config": {"workload": sample, "voxel_views_per_step": nvox},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -449,6 +589,12 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE config number 1..5 (default 4, the target volume)")
+    ap.add_argument("--mode", default="replicas", choices=["replicas", "view-parallel", "block-replicas"],
+                    help="what --gpus N ranks do (DESIGN.md section 10); default: N independent replicas of the OSEM workload")
+    ap.add_argument("--blocked", type=int, default=0, metavar="B", help="config 5 as B^3 blocks + halo (mvd_deconvolve_blocked)")
+    ap.add_argument("--psf-sweep", action="store_true", help="config 5 whole, one record per PSF box 9^3 ... 31x31x63")
+    ap.add_argument("--repeats", type=int, default=2, help="timed repeats of the blocked job (median)")
+    ap.add_argument("--sustained-s", type=float, default=3.0, help="seconds of back-to-back steps for the `sustained` leg (0 = skip)")
     ap.add_argument("--no-graph", action="store_true", help="time plain launches instead of one CUDA graph per iteration")
     ap.add_argument("--e2e-jobs", type=int, default=2)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

@@ -104,6 +104,9 @@ typedef struct {
   void* views_ready;         /* optional cudaEvent_t: mvd_create makes its stream wait for it before the first read of
                               * the views (the initial estimate), so the caller's host-to-device copy of the views
                               * (on another stream) overlaps the PSF precompute.  NULL -> the views are ready. */
+  int block_rank;            /* mvd_deconvolve_blocked only: with block_world > 1 this call processes the blocks whose  */
+  int block_world;           /* index (x fastest, then y, then z) is congruent to block_rank modulo block_world and     */
+                             /* leaves the rest of dst untouched: blocks dealt over GPUs.  0 -> all.    */
 } mvd_options;
 
 /* Fills *opt with the defaults (struct_size set, everything else 0/NULL/defaults). */

@@ -51,6 +51,8 @@ class mvd_options(C.Structure):
         ("n_local", C.c_int),
         ("psi0_value", C.c_float),
         ("views_ready", C.c_void_p),
+        ("block_rank", C.c_int),
+        ("block_world", C.c_int),
     ]
 
 
@@ -372,8 +374,11 @@ class Deconvolver:
 
 
 def deconvolve_blocked(views, psfs, block_dims, iterations, variant="osem", kernel_mode="auto",
-                       halo=None, eps=None, psi_floor=None, literal_product=False, stream=None):
-    """mvd_deconvolve_blocked: block_dims / halo are (x,y,z).  Returns (device tensor, launches)."""
+                       halo=None, eps=None, psi_floor=None, literal_product=False, stream=None,
+                       block_rank=0, block_world=0, out=None):
+    """mvd_deconvolve_blocked: block_dims / halo are (x,y,z).  Returns (device tensor, launches).
+    block_world > 1: only the blocks with index % block_world == block_rank are processed (blocks dealt
+    over GPUs); the other voxels of the result keep what `out` held (zeros if out is None)."""
     import torch
 
     lib = load_library()
@@ -386,6 +391,7 @@ def deconvolve_blocked(views, psfs, block_dims, iterations, variant="osem", kern
     stream = stream if stream is not None else torch.cuda.current_stream(device)
     keep, psf_ptrs, psf_dims = _psf_args(psfs)
     opt = _make_options(kernel_mode, literal_product, eps, psi_floor, None, False)
+    opt.block_rank, opt.block_world = int(block_rank), int(block_world)
     halo_arg = C.cast(_Int3(*halo), C.c_void_p) if halo is not None else None
     nbytes = lib.mvd_blocked_workspace_size(len(views), _Int3(*dims), C.cast(psf_dims, C.c_void_p),
                                             VARIANTS[variant], C.byref(opt), _Int3(*block_dims), halo_arg)
@@ -393,7 +399,12 @@ def deconvolve_blocked(views, psfs, block_dims, iterations, variant="osem", kern
         raise MvdError("mvd_blocked_workspace_size: invalid or unsupported problem")
     with torch.cuda.stream(stream):
         ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
-        dst = torch.empty(shape, dtype=torch.float32, device=device)
+        if out is not None:
+            if tuple(out.shape) != shape or out.dtype != torch.float32 or not out.is_cuda or not out.is_contiguous():
+                raise MvdError("out must be a contiguous CUDA float32 tensor of the views' shape")
+            dst = out
+        else:
+            dst = (torch.zeros if block_world > 1 else torch.empty)(shape, dtype=torch.float32, device=device)
     opt.workspace = (ws.data_ptr() + 255) // 256 * 256
     opt.workspace_bytes = nbytes
     opt.stream = stream.cuda_stream

@@ -150,6 +150,8 @@ static int sm_count() {
 // grid of the grid-stride reduction / fill kernels: 8 CTAs of 256 threads per SM
 static int reduce_blocks() { return 8 * sm_count(); }
 
+constexpr int kMaxZChunks = 64;   // z-chunked schedule: at most this many chunks (one statistics slot each)
+
 static int env_int(const char* name, int dflt) {
   const char* s = getenv(name);
   return (s && *s) ? atoi(s) : dflt;
@@ -335,7 +337,7 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
   P.off_auto = take(kmode == MVD_KERNEL_COMPOUND ? P.auto_stride * sizeof(double) * P.V : 256);
   P.off_stage = take(P.psf_stride * sizeof(float));
   P.sum_blocks = reduce_blocks();
-  P.off_partials = take(sizeof(double) * 2 * (size_t)std::max(P.nctax, P.sum_blocks));
+  P.off_partials = take(sizeof(double) * 2 * (size_t)std::max(P.nctax, P.sum_blocks * kMaxZChunks));
   P.off_scalars = take(sizeof(double) * (size_t)(P.V + 8));
   P.off_cmp = take(sizeof(double) * (6 * 192 + 8));   // mvd_compare partials
   P.total = o;
@@ -362,6 +364,9 @@ struct mvd_ctx {
   bool partial = false;
   float psi0_value = 0.f;
   bool w_valid = false;        // the work buffer holds the x-forward transform of the current psi
+                               // (z-chunked schedule: the x- and y-forward transform)
+  int zchunk = 0;              // > 0: the plane-local passes (y-inverse, x pass, y-forward) run chunk by chunk of this
+                               // many z planes, so a chunk of the work buffer stays in L2 between them
   bool broken = false;
   bool stats_valid = false;
   int stats_ncta = 0;
@@ -646,9 +651,51 @@ mvd_status conv_core(mvd_ctx* c, const float2* in, float2* buf, const float2* sp
   return MVD_OK;
 }
 
+// y-inverse -> x pass (quotient or update) -> y-forward of planes [z0, z0 + nz): all three are local to a z plane
+mvd_status plane_group(mvd_ctx* c, int v, bool update, int z0, int nz, int chunk_index) {
+  const Plan& P = c->P;
+  const int rx = (P.K[v].x - 1) / 2;
+  float2* w = c->W() + (long long)z0 * P.plane;
+  const long long voff = (long long)z0 * P.N[1] * P.N[0];
+  MVD_TRY(y_pass(c, w, +1, nz, false));
+  XArgs a = x_args(c, w, w, rx);
+  a.nrows = (long long)P.N[1] * nz;
+  a.psi = c->psi() + voff;
+  a.partials = c->partials() + 2 * (size_t)chunk_index * P.sum_blocks;
+  if (!update) {
+    a.phi = c->views[v] + voff;
+    MVD_TRY(x_pass(c, a, X_QUOT));
+  } else {
+    a.wts = c->weights.empty() ? nullptr : c->weights[v] + voff;
+    MVD_TRY(x_pass(c, a, a.wts ? X_UPDATE_W : X_UPDATE));
+  }
+  MVD_TRY(y_pass(c, w, -1, nz, false));
+  return MVD_OK;
+}
+
 // one iteration (every view contributes once, L817); requires w_valid
 mvd_status iteration_body(mvd_ctx* c) {
   const Plan& P = c->P;
+  if (!P.combined && c->zchunk > 0) {
+    // eq. 109-112 with the plane-local passes chunked along z: per view  z(H), [y-inv, quotient, y-fwd] per chunk,
+    // z(K), [y-inv, update, y-fwd] per chunk; the work buffer enters and leaves x- and y-transformed
+    const int nchunks = (P.N[2] + c->zchunk - 1) / c->zchunk;
+    for (int v = 0; v < P.V; ++v) {
+      for (int half = 0; half < 2; ++half) {
+        MVD_TRY(z_conv(c, c->W(), c->W(), half ? c->specK(v) : c->specH(v)));
+        if (half == 1 && v == P.V - 1)   // statistics of the last update: one slot of sum_blocks partials per chunk
+          MVD_CK(cudaMemsetAsync(c->partials(), 0, sizeof(double) * 2 * (size_t)nchunks * P.sum_blocks, c->stream), "memset partials");
+        for (int k = 0; k < nchunks; ++k) {
+          // alternate the chunk order so a pass starts on the planes the z pass / previous group wrote last
+          const int kk = (half & 1) ? nchunks - 1 - k : k;
+          const int z0 = kk * c->zchunk, nz = std::min(c->zchunk, P.N[2] - z0);
+          MVD_TRY(plane_group(c, v, half == 1, z0, nz, kk));
+        }
+      }
+    }
+    c->stats_ncta = nchunks * P.sum_blocks;
+    return MVD_OK;
+  }
   if (!P.combined) {
     // eq. 109-112: psi updated after every view, index order (R11)
     for (int v = 0; v < P.V; ++v) {
@@ -683,6 +730,7 @@ mvd_status iteration_body(mvd_ctx* c) {
 mvd_status ensure_w(mvd_ctx* c) {
   if (c->w_valid) return MVD_OK;
   MVD_TRY(x_load(c, c->psi(), c->P.combined ? c->W0() : c->W()));
+  if (!c->P.combined && c->zchunk > 0) MVD_TRY(y_pass(c, c->W(), -1, c->P.N[2], false));
   c->w_valid = true;
   return MVD_OK;
 }
@@ -928,6 +976,8 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
   c->ws = reinterpret_cast<char*>(opt->workspace);
   c->use_graph = opt->use_graph;
   c->use_flip = env_int("MVD_FLIP", 1);
+  c->zchunk = std::max(0, env_int("MVD_ZCHUNK", 0));
+  if (c->zchunk > 0) c->zchunk = std::max(c->zchunk, (c->P.N[2] + kMaxZChunks - 1) / kMaxZChunks);
   if (c->use_graph && !c->stream) {   // the legacy default stream cannot be captured
     fprintf(stderr, "mvd_create: use_graph needs a non-default stream\n");
     delete c;
@@ -1322,6 +1372,8 @@ extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* vi
   const mvd_options* opt = defaults(opt_in, &tmp);
   if (opt->weights || opt->views_ready || opt->local_views || opt->psi0 || opt->psi0_value != 0.f)
     return MVD_ERR_UNSUPPORTED;   // whole-volume options
+  const int bworld = opt->block_world > 1 ? opt->block_world : 1;
+  if (opt->block_rank < 0 || opt->block_rank >= bworld) return MVD_ERR_INVALID_ARG;
   BlockedLayout L;
   mvd_status s = blocked_layout(L, n_views, dims, psf_dims, variant, opt, block_dims, halo);
   if (s != MVD_OK) return s;
@@ -1356,8 +1408,21 @@ extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* vi
   bool have_kern = false;
   for (const auto& shape : L.shapes) {
     const int d[3] = {shape[0], shape[1], shape[2]};
+    // blocks of this shape that belong to this rank (blocks dealt round-robin by index, L225)
+    bool mine = false;
+    {
+      long long idx = 0;
+      for (const Seg& sz : L.seg[2])
+        for (const Seg& sy : L.seg[1])
+          for (const Seg& sx : L.seg[0]) {
+            if (sx.e1 - sx.e0 == d[0] && sy.e1 - sy.e0 == d[1] && sz.e1 - sz.e0 == d[2] && idx % bworld == opt->block_rank) mine = true;
+            ++idx;
+          }
+    }
+    if (!mine) continue;
     mvd_options o = *opt;
     o.fft_dims[0] = o.fft_dims[1] = o.fft_dims[2] = 0;
+    o.block_rank = o.block_world = 0;
     o.psi0 = psi0;
     o.workspace = ws + L.off_ctx;
     o.workspace_bytes = L.ctx_bytes;
@@ -1375,10 +1440,13 @@ extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* vi
     const Dims3 E{d[0], d[1], d[2]};
     const long long ext = (long long)d[0] * d[1] * d[2];
     const unsigned grid = (unsigned)std::min<long long>((ext + 255) / 256, (long long)nb * 8);
+    long long bidx = -1;
     for (const Seg& sz : L.seg[2])
       for (const Seg& sy : L.seg[1])
         for (const Seg& sx : L.seg[0]) {
+          ++bidx;
           if (sx.e1 - sx.e0 != d[0] || sy.e1 - sy.e0 != d[1] || sz.e1 - sz.e0 != d[2]) continue;
+          if (bidx % bworld != opt->block_rank) continue;
           for (int v = 0; v < n_views; ++v) {
             gather_block_kernel<<<grid, 256, 0, st>>>(views[v], N, Dims3{sx.e0, sy.e0, sz.e0}, E,
                                                       const_cast<float*>(bviews[v]));

@@ -338,6 +338,32 @@ def test_blocked_matches_blocked_oracle(mvd):
     assert launches > 0
 
 
+def test_blocked_blocks_dealt_over_two_ranks(mvd):
+    """PAPER.md L225 (blocks on two GPUs): block_world = 2 deals the blocks round-robin; the two ranks' calls write
+    disjoint blocks of one result, together bit-identical to the single call; each leaves the other's blocks alone."""
+    import torch
+    p = mvd_synth.make_problem(1, dims=(48, 40, 36), psf_dims=(7, 7, 11))
+    block = (20, 24, 16)
+    views = to_dev(p.views)
+    whole, _ = mvd.deconvolve_blocked(views, p.psfs, block, 2, variant="osem")
+    out = torch.full_like(whole, -1.0)
+    r0, l0 = mvd.deconvolve_blocked(views, p.psfs, block, 2, variant="osem", block_rank=0, block_world=2, out=out)
+    assert r0 is out
+    part = out.cpu().numpy()
+    assert (part == -1.0).any() and (part != -1.0).any()                 # rank 0 wrote its blocks only
+    nb = [-(-n // b) for n, b in zip((48, 40, 36), block)]               # blocks per axis (x, y, z)
+    for iz in range(nb[2]):
+        for iy in range(nb[1]):
+            for ix in range(nb[0]):
+                idx = (iz * nb[1] + iy) * nb[0] + ix
+                blk = part[iz * block[2]:(iz + 1) * block[2], iy * block[1]:(iy + 1) * block[1], ix * block[0]:(ix + 1) * block[0]]
+                assert ((blk == -1.0).all() if idx % 2 else (blk != -1.0).all()), (ix, iy, iz)
+    _, l1 = mvd.deconvolve_blocked(views, p.psfs, block, 2, variant="osem", block_rank=1, block_world=2, out=out)
+    assert torch.equal(out, whole) and l0 > 0 and l1 > 0
+    with pytest.raises(mvd.MvdError):
+        mvd.deconvolve_blocked(views, p.psfs, block, 2, variant="osem", block_rank=2, block_world=2)
+
+
 def test_blocked_single_block_equals_whole(mvd, tiny):
     got, _ = mvd.deconvolve_blocked(to_dev(tiny.views), tiny.psfs, (64, 64, 64), 2, variant="efficient")
     whole, _ = gpu_checkpoints(mvd, tiny, "efficient", "auto", (2,))
