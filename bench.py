@@ -345,7 +345,7 @@ def run_ours(args):
         return emit(line)
 
     # ============================ block-wise processing (config 5) ============================
-    if args.blocked or args.mode == "block-replicas":
+    if (args.blocked and not args.psf_sweep) or args.mode == "block-replicas":
         # R13 / PAPER.md L943, L225: 256^3 blocks + halo r, every block an independent problem; with several ranks
         # the blocks are dealt round-robin (the paper's two-GPU mode) and no rank talks to another
         B = args.blocked or 256
@@ -387,6 +387,25 @@ def run_ours(args):
         sweep = []
         for box in SWEEP_BOXES:
             psfs = sweep_psfs(k, box)
+            if args.blocked:
+                # the same sweep in block-wise mode, where the PSF half-size sets the halo and so the overhead (L240)
+                B, iters, reps = args.blocked, prob.iterations, []
+                for rep in range(2):                                   # first pass = warm-up
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    barrier()
+                    e0.record(stream)
+                    out, _ = mvd.deconvolve_blocked(dev_views, psfs, (B, B, B), iters, variant="osem", stream=stream)
+                    e1.record(stream)
+                    barrier()
+                    reps.append(e0.elapsed_time(e1))
+                    del out
+                halo = [(b - 1) // 2 for b in box]
+                ext = float(np.prod([B + 2 * h for h in halo])) / B ** 3
+                sweep.append({"psf_box": list(box), "block": B, "halo": halo, "iterations": iters, "ms_total": reps[-1],
+                              "ms_per_step": reps[-1] / iters, "value": nvox * V * iters / (reps[-1] * 1e-3) / 1e9,
+                              "extended_over_central_voxels_interior_block": ext})
+                log("[bench] blocked sweep %s: %.1f ms" % (box, reps[-1]))
+                continue
             d = mvd.Deconvolver(dev_views, psfs, variant="osem", stream=stream, use_graph=True)
             for _ in range(args.warmup):
                 d.iterate(1)
@@ -406,8 +425,9 @@ def run_ours(args):
             torch.cuda.empty_cache()
         ref = [r for r in sweep if tuple(r["psf_box"]) == tuple(prob.psf_dims)] or sweep[-1:]
         line = dict(base, value=ref[0]["value"], ms_per_step=ref[0]["ms_per_step"], scaling="weak",
-                    config={"workload": wl + " swept over PSF boxes 9^3 ... 31x31x63, efficient-OSEM, whole volume; `value` is the "
-                                             "%dx%dx%d record" % tuple(ref[0]["psf_box"]), "cuda_graph": True,
+                    config={"workload": wl + " swept over PSF boxes 9^3 ... 31x31x63, efficient-OSEM, %s; `value` is the "
+                                             "%dx%dx%d record" % (("as %d^3 blocks + halo r" % args.blocked) if args.blocked else "whole volume",
+                                                                  *ref[0]["psf_box"]), "cuda_graph": not args.blocked,
                             "l2": "inputs larger than L2", "parallelism": "single GPU"},
                     clocks=sampler.summary(0, time.perf_counter()), gpu_launches=None, e2e=None, roofline=None, sweep=sweep,
                     peak_source=peak_src)

@@ -19,6 +19,7 @@
  *       MVD_INDEPENDENT  psi <- max(psi * (prod_v max(f_v,0))^(1/V), psi_floor), K = PLAIN     (eq. 70; root: eq. 44, R1)
  *       MVD_EFFICIENT    same combination, K = COMPOUND                                        (eq. 104)
  *   One iteration = every view has contributed once (footnote L817).
+ *   Options: per-view weights (section 12), Tikhonov regularisation (L64, L869): see mvd_options.
  *
  * Memory conventions
  *   - Volumes are fp32, x fastest: element (x,y,z) at [(z*Ny + y)*Nx + x].  dims = {Nx,Ny,Nz}.
@@ -104,6 +105,11 @@ typedef struct {
   void* views_ready;         /* optional cudaEvent_t: mvd_create makes its stream wait for it before the first read of
                               * the views (the initial estimate), so the caller's host-to-device copy of the views
                               * (on another stream) overlaps the PSF precompute.  NULL -> the views are ready. */
+  float tikhonov_lambda;     /* >= 0; 0 = off.  Tikhonov regularisation of every psi update (ref. 20; the
+                              * paper prints no formula: reading R14 of DESIGN.md).  With u the unregularised new value
+                              * (psi*f_v, or psi*(prod f_v)^(1/V)), the update stores the positive root of
+                              * (lambda/2) psi^2 + psi - u = 0, psi = 2u / (1 + sqrt(1 + 2 lambda u)), then applies the floor:
+                              * the EM M-step for the Poisson likelihood with the penalty (lambda/4) sum psi^2.           */
   int block_rank;            /* mvd_deconvolve_blocked only: with block_world > 1 this call processes the blocks whose  */
   int block_world;           /* index (x fastest, then y, then z) is congruent to block_rank modulo block_world and     */
                              /* leaves the rest of dst untouched: blocks dealt over GPUs.  0 -> all.    */

@@ -17,6 +17,8 @@ What it computes (PAPER.md line numbers; "R<n>" = reading listed in DESIGN.md):
 * eq. 107 / 108 (L748, L755): optimisation I / II back-projectors.
 * eq. 109-112 (L769-776), eq. 114-117 (L786-793): sequential (OSEM) schedule.
 * eq. 44 (L455) + L464: the combined update takes the |V|-th root (R1).
+* L64, L869 + ref. 20: optional Tikhonov regularisation of every update (R14; the paper prints no
+  formula, see ``tikhonov`` below: parity unpinned by the paper).
 
 Arrays are numpy, shape (Nz, Ny, Nx), x fastest.  All arithmetic is float64.
 
@@ -182,6 +184,20 @@ def initial_estimate(views):
     return np.full(np.asarray(views[0]).shape, tot / cnt)
 
 
+def tikhonov(u, lam):
+    """Tikhonov-regularised value of an update (L64 "option for Tikhonov regularization", L869, ref. 20).
+
+    PAPER.md gives no formula (reading R14).  Used here: the EM M-step for the Poisson likelihood with the
+    quadratic (Tikhonov) penalty (lam/4) * sum psi^2.  With u = psi^r * f the unpenalised update, the new
+    estimate maximises  u log(psi) - psi - (lam/4) psi^2  per voxel:  u/psi - 1 - (lam/2) psi = 0, i.e. it is
+    the positive root of  (lam/2) psi^2 + psi - u = 0:
+        psi = (sqrt(1 + 2 lam u) - 1) / lam  =  2 u / (1 + sqrt(1 + 2 lam u))     (second form: no cancellation)
+    lam = 0 leaves u unchanged; psi < u for lam > 0 ("slows down convergence", L869)."""
+    if lam == 0.0:
+        return u
+    return 2.0 * u / (1.0 + np.sqrt(1.0 + 2.0 * lam * u))
+
+
 def rl_factor(psi, phi, p, k, eps=EPS_DEFAULT, backend="fft"):
     """f_v = (phi_v / (psi * P_v)) * K_v (eq. 1, eq. 13, EM description L306)."""
     same = _same(backend)
@@ -197,7 +213,8 @@ class Oracle:
     """
 
     def __init__(self, views, psfs, variant="osem", kernel_mode="auto", literal_product=False,
-                 eps=EPS_DEFAULT, psi_floor=FLOOR_DEFAULT, psi0=None, backend="fft", weights=None):
+                 eps=EPS_DEFAULT, psi_floor=FLOOR_DEFAULT, psi0=None, backend="fft", weights=None,
+                 tikhonov_lambda=0.0):
         if variant not in VARIANTS:
             raise ValueError(variant)
         if weights is not None and variant != "osem":
@@ -215,6 +232,9 @@ class Oracle:
         self.eps = float(eps)
         self.psi_floor = float(psi_floor)
         self.backend = backend
+        self.tikhonov_lambda = float(tikhonov_lambda)
+        if self.tikhonov_lambda < 0.0:
+            raise ValueError("tikhonov_lambda must be >= 0")
         self.kernels = [back_projector(self.psfs, v, self.kernel_mode, backend)
                         for v in range(len(self.psfs))]
         self.weights = None if weights is None else [np.asarray(w, dtype=np.float64) for w in weights]
@@ -242,7 +262,7 @@ class Oracle:
             # suggested by a Lucy-Richardson update step that will be applied":
             # psi*f = psi + (psi*f - psi)  ->  psi + w*(psi*f - psi) = psi*(1 + w*(f - 1))
             f = 1.0 + self.weights[v] * (f - 1.0)
-        self._commit(np.maximum(self.psi * f, self.psi_floor))
+        self._commit(np.maximum(tikhonov(self.psi * f, self.tikhonov_lambda), self.psi_floor))
         return self.psi
 
     def iterate(self, n=1):
@@ -260,7 +280,7 @@ class Oracle:
                     prod *= f if self.literal_product else np.maximum(f, 0.0)
                 if not self.literal_product:
                     prod = prod ** (1.0 / nv)       # eq. 44: geometric mean (R1)
-                self._commit(np.maximum(self.psi * prod, self.psi_floor))
+                self._commit(np.maximum(tikhonov(self.psi * prod, self.tikhonov_lambda), self.psi_floor))
             self.iterations_done += 1
         return self.psi
 

@@ -51,6 +51,7 @@ class mvd_options(C.Structure):
         ("n_local", C.c_int),
         ("psi0_value", C.c_float),
         ("views_ready", C.c_void_p),
+        ("tikhonov_lambda", C.c_float),
         ("block_rank", C.c_int),
         ("block_world", C.c_int),
     ]
@@ -148,7 +149,7 @@ def _psf_args(psfs):
     return arrs, ptrs, dims
 
 
-def _make_options(kernel_mode, literal_product, eps, psi_floor, fft_dims, use_graph):
+def _make_options(kernel_mode, literal_product, eps, psi_floor, fft_dims, use_graph, tikhonov_lambda=None):
     lib = load_library()
     opt = mvd_options()
     lib.mvd_options_init(C.byref(opt))
@@ -161,6 +162,8 @@ def _make_options(kernel_mode, literal_product, eps, psi_floor, fft_dims, use_gr
     if fft_dims is not None:
         opt.fft_dims[:] = [int(x) for x in fft_dims]
     opt.use_graph = int(bool(use_graph))
+    if tikhonov_lambda is not None:
+        opt.tikhonov_lambda = float(tikhonov_lambda)
     return opt
 
 
@@ -189,7 +192,7 @@ class Deconvolver:
 
     def __init__(self, views, psfs, variant="osem", kernel_mode="auto", literal_product=False,
                  eps=None, psi_floor=None, psi0=None, fft_dims=None, use_graph=False, stream=None,
-                 weights=None, views_ready=None, local_views=None, psi0_value=None):
+                 weights=None, views_ready=None, local_views=None, psi0_value=None, tikhonov_lambda=None):
         import torch
 
         lib = load_library()
@@ -222,7 +225,7 @@ class Deconvolver:
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._psfs, psf_ptrs, psf_dims = _psf_args(psfs)
         self._psf_dims = psf_dims
-        opt = _make_options(kernel_mode, literal_product, eps, psi_floor, fft_dims, use_graph)
+        opt = _make_options(kernel_mode, literal_product, eps, psi_floor, fft_dims, use_graph, tikhonov_lambda)
         if local_views is not None:
             opt.local_views = C.cast(self._local, C.c_void_p)
             opt.n_local = len(local_views)
@@ -375,7 +378,7 @@ class Deconvolver:
 
 def deconvolve_blocked(views, psfs, block_dims, iterations, variant="osem", kernel_mode="auto",
                        halo=None, eps=None, psi_floor=None, literal_product=False, stream=None,
-                       block_rank=0, block_world=0, out=None):
+                       block_rank=0, block_world=0, out=None, tikhonov_lambda=None):
     """mvd_deconvolve_blocked: block_dims / halo are (x,y,z).  Returns (device tensor, launches).
     block_world > 1: only the blocks with index % block_world == block_rank are processed (blocks dealt
     over GPUs); the other voxels of the result keep what `out` held (zeros if out is None)."""
@@ -390,7 +393,7 @@ def deconvolve_blocked(views, psfs, block_dims, iterations, variant="osem", kern
     device = views[0].device
     stream = stream if stream is not None else torch.cuda.current_stream(device)
     keep, psf_ptrs, psf_dims = _psf_args(psfs)
-    opt = _make_options(kernel_mode, literal_product, eps, psi_floor, None, False)
+    opt = _make_options(kernel_mode, literal_product, eps, psi_floor, None, False, tikhonov_lambda)
     opt.block_rank, opt.block_world = int(block_rank), int(block_world)
     halo_arg = C.cast(_Int3(*halo), C.c_void_p) if halo is not None else None
     nbytes = lib.mvd_blocked_workspace_size(len(views), _Int3(*dims), C.cast(psf_dims, C.c_void_p),

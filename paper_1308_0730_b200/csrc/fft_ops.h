@@ -108,6 +108,7 @@ struct XArgs {
   float* acc;              // X_ACCUM: product accumulator / raw destination
   double* partials;        // per-CTA {flux, l1} (X_UPDATE, ACC_LAST)
   float eps, psi_floor, inv_nviews;
+  float tikhonov;          // lambda of the Tikhonov-regularised update (0 = off), see mvd.h
   int acc_mode;            // AccMode
   int literal_product;
   int complex_in;          // X_LOAD: rows of `in` are complex and transformed in full

@@ -237,7 +237,8 @@ __global__ void fill_value_kernel(float* __restrict__ a, long long n, float valu
 // max(f_v, 0) over ALL views; psi <- max(psi * acc^(1/V), floor); per-block {sum psi, sum |dpsi|}
 __global__ void __launch_bounds__(256) apply_product_kernel(float* __restrict__ psi, const float* __restrict__ acc,
                                                             long long n, float inv_nviews, int literal,
-                                                            float psi_floor, double* __restrict__ partials) {
+                                                            float psi_floor, float tikhonov,
+                                                            double* __restrict__ partials) {
   __shared__ double red[32];
   double flux = 0.0, l1 = 0.0;
   const long long stride = (long long)gridDim.x * blockDim.x;
@@ -245,7 +246,9 @@ __global__ void __launch_bounds__(256) apply_product_kernel(float* __restrict__ 
     float f = acc[i];
     if (!literal && inv_nviews != 1.f) f = powf(f, inv_nviews);
     const float o = psi[i];
-    const float nw = fmaxf(o * f, psi_floor);
+    float u = o * f;
+    if (tikhonov > 0.f) u = __fdiv_rn(2.f * u, 1.f + __fsqrt_rn(fmaf(2.f * tikhonov, u, 1.f)));   // mvd.h, R14
+    const float nw = fmaxf(u, psi_floor);
     psi[i] = nw;
     flux += nw;
     l1 += fabsf(nw - o);

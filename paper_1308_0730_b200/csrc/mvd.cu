@@ -355,7 +355,7 @@ struct mvd_ctx {
   Plan P;
   mvd_variant variant = MVD_OSEM;
   int literal = 0;
-  float eps = 1e-6f, psi_floor = 1e-6f;
+  float eps = 1e-6f, psi_floor = 1e-6f, tikhonov = 0.f;
   cudaStream_t stream = nullptr;
   char* ws = nullptr;
   std::vector<const float*> views;
@@ -594,6 +594,7 @@ XArgs x_args(mvd_ctx* c, const float2* in, float2* out, int rx) {
   a.nx = P.N[0]; a.hx = P.hx; a.rx = rx;
   a.psi = c->psi(); a.acc = c->acc(); a.partials = c->partials();
   a.eps = c->eps; a.psi_floor = c->psi_floor; a.inv_nviews = 1.0f / (float)P.V;
+  a.tikhonov = c->tikhonov;
   a.literal_product = c->literal;
   return a;
 }
@@ -972,6 +973,8 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
   c->literal = opt->literal_product ? 1 : 0;
   c->eps = opt->eps > 0.f ? opt->eps : 1e-6f;
   c->psi_floor = opt->psi_floor >= 0.f ? opt->psi_floor : 1e-6f;
+  if (!(opt->tikhonov_lambda >= 0.f) || !std::isfinite(opt->tikhonov_lambda)) { delete c; return MVD_ERR_INVALID_ARG; }
+  c->tikhonov = opt->tikhonov_lambda;
   c->stream = reinterpret_cast<cudaStream_t>(opt->stream);
   c->ws = reinterpret_cast<char*>(opt->workspace);
   c->use_graph = opt->use_graph;
@@ -1129,7 +1132,7 @@ mvd_status mvd_apply_product(mvd_ctx* c, int total_views) {
   const Plan& P = c->P;
   if (!P.combined) return MVD_ERR_UNSUPPORTED;
   apply_product_kernel<<<P.sum_blocks, 256, 0, c->stream>>>(c->psi(), c->acc(), P.nvox, 1.0f / (float)total_views,
-                                                          c->literal, c->psi_floor, c->partials());
+                                                          c->literal, c->psi_floor, c->tikhonov, c->partials());
   MVD_CK(cudaGetLastError(), "apply_product_kernel");
   ++c->launches;
   c->w_valid = false;

@@ -38,6 +38,12 @@ struct PassCfg {
 
 MVD_DEV float2 ld_tw(const float2* tw, int idx) { return __ldg(tw + idx); }
 
+// Tikhonov-regularised value of an update u (mvd.h, R14): positive root of (lam/2) psi^2 + psi - u = 0
+// in the cancellation-free form; lam = 0 returns u itself
+MVD_DEV float tikhonov_update(float u, float lam) {
+  return lam > 0.f ? __fdiv_rn(2.f * u, 1.f + __fsqrt_rn(fmaf(2.f * lam, u, 1.f))) : u;
+}
+
 // =========================================================================================
 // strided pencil FFT, form F, direction DIR (-1 forward, +1 inverse; unnormalised)
 // =========================================================================================
@@ -287,14 +293,14 @@ xrow_kernel(const XArgs p) {
             if (has_b) z.y = p.phi[ib] / fmaxf(vb, p.eps);
           } else if constexpr (MODE == X_UPDATE) {
             const float o = p.psi[it];
-            const float nw = fmaxf(o * vt, p.psi_floor);
+            const float nw = fmaxf(tikhonov_update(o * vt, p.tikhonov), p.psi_floor);
             p.psi[it] = nw;
             flux += nw;
             l1 += fabsf(nw - o);
             z.x = nw;
             if (has_b) {
               const float o2 = p.psi[ib];
-              const float nw2 = fmaxf(o2 * vb, p.psi_floor);
+              const float nw2 = fmaxf(tikhonov_update(o2 * vb, p.tikhonov), p.psi_floor);
               p.psi[ib] = nw2;
               flux += nw2;
               l1 += fabsf(nw2 - o2);
@@ -320,14 +326,14 @@ xrow_kernel(const XArgs p) {
                   fb = powf(fb, p.inv_nviews);
                 }
                 const float o = p.psi[it];
-                const float nw = fmaxf(o * ft, p.psi_floor);
+                const float nw = fmaxf(tikhonov_update(o * ft, p.tikhonov), p.psi_floor);
                 p.psi[it] = nw;
                 flux += nw;
                 l1 += fabsf(nw - o);
                 z.x = nw;
                 if (has_b) {
                   const float o2 = p.psi[ib];
-                  const float nw2 = fmaxf(o2 * fb, p.psi_floor);
+                  const float nw2 = fmaxf(tikhonov_update(o2 * fb, p.tikhonov), p.psi_floor);
                   p.psi[ib] = nw2;
                   flux += nw2;
                   l1 += fabsf(nw2 - o2);

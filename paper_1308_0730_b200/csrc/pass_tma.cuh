@@ -188,7 +188,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
         } else if constexpr (MODE == X_UPDATE || MODE == X_UPDATE_W) {
           const float o = rrow[x];
           if (has_w) v = fmaf(wrow[x], v - 1.f, 1.f);                     // section 12: fraction w of the RL step
-          const float nw = fmaxf(o * v, p.psi_floor);                     // eq. 109-112, R4
+          const float nw = fmaxf(tikhonov_update(o * v, p.tikhonov), p.psi_floor);   // eq. 109-112, R4, R14
           prow[x] = nw;
           flux += nw;
           l1 += fabsf(nw - o);
@@ -202,7 +202,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
           }
           if (!p.literal_product && p.inv_nviews != 1.f) f = powf(f, p.inv_nviews);
           const float o = prow[x];
-          const float nw = fmaxf(o * f, p.psi_floor);
+          const float nw = fmaxf(tikhonov_update(o * f, p.tikhonov), p.psi_floor);
           prow[x] = nw;
           flux += nw;
           l1 += fabsf(nw - o);

@@ -536,6 +536,53 @@ def test_weighted_config2_size(mvd, config2):
 
 
 # ------------------------------------------------------------------------------------------
+# Tikhonov regularisation (L64, L869; R14): fused into the update kernels, zero extra bytes
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", ["osem", "efficient", "independent"])
+def test_tikhonov_matches_oracle(mvd, tiny, variant):
+    for lam in (0.006, 0.06):                                       # values of the paper's sweep (L145)
+        g, st = gpu_checkpoints(mvd, tiny, variant, "auto", (1, 5), tikhonov_lambda=lam)
+        o, orc = oracle_checkpoints(tiny, variant, "auto", (1, 5), tikhonov_lambda=lam)
+        check(g[1], o[1], 1, "tikhonov %s %g" % (variant, lam))
+        check(g[5], o[5], 5, "tikhonov %s %g" % (variant, lam))
+        assert st["flux"] == pytest.approx(orc.flux, rel=1e-5)
+    plain, _ = gpu_checkpoints(mvd, tiny, variant, "auto", (2,))
+    zero, _ = gpu_checkpoints(mvd, tiny, variant, "auto", (2,), tikhonov_lambda=0.0)
+    assert np.array_equal(plain[2], zero[2])                        # lambda = 0: the unregularised path, bit for bit
+    reg, _ = gpu_checkpoints(mvd, tiny, variant, "auto", (2,), tikhonov_lambda=0.06)
+    assert reg[2].sum(dtype=np.float64) < plain[2].sum(dtype=np.float64)
+    with pytest.raises(mvd.MvdError):
+        gpu_checkpoints(mvd, tiny, variant, "auto", (1,), tikhonov_lambda=-0.5)
+
+
+def test_tikhonov_config2_size_with_weights_blocks_and_view_parallel(mvd, config2, tiny):
+    """lambda = 0.006 (the paper's real-data value, Suppl. Table 1) at 128^3 under graph replay; with section-12
+    weights; in block-wise mode; and through the view-parallel calls (apply_product_kernel)."""
+    import torch
+    lam = 0.006
+    g, _ = gpu_checkpoints(mvd, config2, "osem", "auto", (1, 10), tikhonov_lambda=lam, use_graph=True)
+    o, _ = oracle_checkpoints(config2, "osem", "auto", (1, 10), tikhonov_lambda=lam)
+    check(g[1], o[1], 1, "tikhonov config 2")
+    check(g[10], o[10], 10, "tikhonov config 2")
+    ws = _partial_overlap_weights(tiny.views[0].shape, 3)
+    wdev = [torch.from_numpy(w.astype(np.float32)).cuda() for w in ws]
+    w32 = [w.astype(np.float32).astype(np.float64) for w in ws]
+    g, _ = gpu_checkpoints(mvd, tiny, "osem", "auto", (3,), tikhonov_lambda=lam, weights=wdev)
+    o, _ = oracle_checkpoints(tiny, "osem", "auto", (3,), tikhonov_lambda=lam, weights=w32)
+    check(g[3], o[3], 3, "tikhonov + weights")
+    p = mvd_synth.make_problem(1, dims=(48, 40, 36), psf_dims=(7, 7, 11))
+    got, _ = mvd.deconvolve_blocked(to_dev(p.views), p.psfs, (20, 24, 16), 3, variant="osem", tikhonov_lambda=lam)
+    ref = O.deconvolve_blocked(p.views, p.psfs, (16, 24, 20), "osem", 3, tikhonov_lambda=lam)
+    check(got.cpu().numpy(), ref, 3, "tikhonov blocked")
+    d = mvd.ViewParallelDeconvolver(to_dev(tiny.views), tiny.psfs, variant="efficient", tikhonov_lambda=lam)
+    d.iterate(2)
+    orc = O.Oracle(tiny.views, tiny.psfs, "efficient", tikhonov_lambda=lam)
+    orc.iterate(2)
+    check(d.get_estimate_host(), orc.psi, 2, "tikhonov view-parallel")
+    d.close()
+
+
+# ------------------------------------------------------------------------------------------
 # view-parallel combined variants (L815; SURVEY 8(e)/8(f) NEXT-4): two "ranks" emulated on one GPU as two
 # contexts that own different views; their partial products are multiplied as the all-reduce would
 # ------------------------------------------------------------------------------------------

@@ -371,6 +371,54 @@ def test_view_update_is_the_osem_step():
 
 
 # --------------------------------------------------------------------------------------
+# Tikhonov regularisation (L64, L869, ref. 20; reading R14: no formula in PAPER.md -> parity unpinned by the
+# paper; what is pinned here is that the oracle computes the penalised M-step it documents)
+# --------------------------------------------------------------------------------------
+def test_tikhonov_update_solves_the_penalised_m_step(tiny):
+    """With u the unregularised update, the regularised one is the positive root of (lam/2) psi^2 + psi - u = 0,
+    i.e. the stationary point of u log(psi) - psi - (lam/4) psi^2 per voxel; checked from the UNREGULARISED oracle's
+    update (so a wrong factor, sign or a regularisation applied to f instead of psi*f fails)."""
+    rng = np.random.default_rng(11)
+    psi0 = rng.random(tiny.views[0].shape) * 80 + 1
+    for variant in ("osem", "efficient"):
+        plain = O.Oracle(tiny.views[:1] if variant == "osem" else tiny.views, tiny.psfs[:1] if variant == "osem" else tiny.psfs,
+                         variant, psi0=psi0)
+        plain.iterate(1)
+        u = plain.psi                                              # psi0 * f (osem, V = 1) / psi0 * (prod f)^(1/V)
+        for lam in (0.0006, 0.006, 0.06, 2.0):                     # the paper's values (L145, L151) and a large one
+            reg = O.Oracle(plain.views, [p.copy() for p in plain.psfs], variant, psi0=psi0, tikhonov_lambda=lam)
+            reg.iterate(1)
+            r = reg.psi
+            assert np.allclose(0.5 * lam * r * r + r, u, rtol=1e-12, atol=0)          # the quadratic
+            assert np.allclose(u / r - 1.0 - 0.5 * lam * r, 0.0, atol=1e-10)         # the stationarity condition
+            assert np.all(r > 0) and np.all(r < u)                                    # damped, positive
+            assert np.allclose(r, (np.sqrt(1 + 2 * lam * u) - 1) / lam, rtol=1e-9)    # the textbook root formula
+    # closed values: u = 4, lam = 1/2 -> psi^2/4 + psi - 4 = 0 -> psi = 2(sqrt(5) - 1)
+    assert O.tikhonov(np.array([4.0]), 0.5)[0] == pytest.approx(2 * (np.sqrt(5.0) - 1), rel=1e-15)
+    assert O.tikhonov(np.array([1.5]), 1.0)[0] == pytest.approx(1.0, rel=1e-15)        # psi^2/2 + psi - 3/2 = 0 -> psi = 1
+
+
+def test_tikhonov_zero_lambda_is_the_plain_update_and_lambda_orders_the_flux(tiny):
+    a = O.deconvolve(tiny.views, tiny.psfs, "osem", 3)
+    b = O.deconvolve(tiny.views, tiny.psfs, "osem", 3, tikhonov_lambda=0.0)
+    assert np.array_equal(a, b)
+    c = O.deconvolve(tiny.views, tiny.psfs, "osem", 3, tikhonov_lambda=1e-12)
+    assert np.allclose(a, c, rtol=1e-7)                           # lam*u/2 ~ 1e-10 per update, amplified by the iteration
+    # first order in lambda: psi = u - lam u^2 / 2 + O(lam^2)
+    u = np.array([0.5, 3.0, 40.0])
+    lam = 1e-6
+    assert np.allclose(O.tikhonov(u, lam), u - 0.5 * lam * u * u, rtol=1e-9)
+    flux = []
+    for lam in (0.0, 0.0006, 0.006, 0.06):
+        o = O.Oracle(tiny.views, tiny.psfs, "osem", tikhonov_lambda=lam)
+        o.iterate(2)
+        flux.append(o.flux)
+    assert all(y < x for x, y in zip(flux, flux[1:]))              # more regularisation, less flux
+    with pytest.raises(ValueError):
+        O.Oracle(tiny.views, tiny.psfs, "osem", tikhonov_lambda=-1.0)
+
+
+# --------------------------------------------------------------------------------------
 # section 12 (L891-903): weights of partially overlapping views
 # --------------------------------------------------------------------------------------
 def test_weights_interpolate_between_old_estimate_and_rl_step(tiny):
