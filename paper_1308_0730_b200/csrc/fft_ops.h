@@ -134,7 +134,8 @@ struct LengthOps {
   // TMA-staged passes (pass_tma.cuh)
   cudaError_t (*xrow_tma)(const XArgs&, int mode, cudaStream_t);
   size_t (*xrow_tma_smem)(int rows, int rx, int nx, int weighted);
-  int (*xrow_tma_blocks_per_sm)(int mode, int nthreads, size_t smem);
+  int (*xrow_tma_blocks_per_sm)(int mode, int flags, int nthreads, size_t smem);
+  int (*xrow_tma_flags)(const XArgs&, int mode);   // compile-time variant of the kernel this launch selects
   cudaError_t (*strided_tma)(const StridedTmaArgs&, int dir, cudaStream_t);
   size_t (*strided_tma_smem)(int T, int boxr, int nbox, int nst);
   int (*strided_tma_blocks_per_sm)(int dir, int nthreads, size_t smem);

@@ -21,6 +21,6 @@ cudaError_t init_all() {
 }  // namespace
 const LengthOps MVD_CAT(ops_, MVD_INST_A, _, MVD_INST_B) = {
     L::Cfg::M, MVD_INST_A, MVD_INST_B, L::Cfg::MAX_THREADS, &init_all, &L::strided, &L::zconv, &L::xrow,
-    &L::strided_smem, &L::xrow_smem, &LT::xrow, &LT::xrow_smem, &LT::xrow_blocks_per_sm,
+    &L::strided_smem, &L::xrow_smem, &LT::xrow, &LT::xrow_smem, &LT::xrow_blocks_per_sm, &LT::xrow_flags_of,
     &LT::strided, &LT::strided_smem, &LT::strided_blocks_per_sm, &LT::zconv, &LT::zconv_smem, &LT::zconv_blocks_per_sm};
 }  // namespace mvd

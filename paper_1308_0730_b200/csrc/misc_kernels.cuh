@@ -88,6 +88,15 @@ __global__ void __launch_bounds__(1024) normalise_kernel(const Tin* __restrict__
 
 struct Dims3 { int x, y, z; };
 
+// tw[j] = exp(-2*pi*i*j/M), evaluated in double (sincospi is exact at the multiples of a quarter turn)
+__global__ void twiddle_kernel(float2* __restrict__ tw, int M) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= M) return;
+  double s, c;
+  sincospi(-2.0 * (double)j / (double)M, &s, &c);
+  tw[j] = make_float2((float)c, (float)s);
+}
+
 // a[m] = (P (*) flip P)[m] = sum_u P[u] P[u + K-1-m], m in [0, 2K-1) per axis   (P_w (*) P_w*)
 __global__ void __launch_bounds__(128) autocorr_kernel(const double* __restrict__ P, Dims3 K,
                                                        double* __restrict__ a) {
@@ -247,7 +256,12 @@ __global__ void __launch_bounds__(256) apply_product_kernel(float* __restrict__ 
     if (!literal && inv_nviews != 1.f) f = powf(f, inv_nviews);
     const float o = psi[i];
     float u = o * f;
-    if (tikhonov > 0.f) u = __fdiv_rn(2.f * u, 1.f + __fsqrt_rn(fmaf(2.f * tikhonov, u, 1.f)));   // mvd.h, R14
+    if (tikhonov > 0.f) {                                      // mvd.h, R14 (same arithmetic as tikhonov_value of the x pass)
+      const float t = fmaf(2.f * tikhonov, u, 1.f);
+      float r;
+      asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(t));
+      asm("div.approx.ftz.f32 %0, %1, %2;" : "=f"(u) : "f"(2.f * u), "f"(fmaf(t, r, 1.f)));
+    }
     const float nw = fmaxf(u, psi_floor);
     psi[i] = nw;
     flux += nw;

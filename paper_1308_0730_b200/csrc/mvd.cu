@@ -92,7 +92,7 @@ struct Plan {
   int ztma = 0, Tzt = 0, ntzt = 0, zbox = 0, znbox = 0, znst = 2;
   // workspace offsets (bytes)
   size_t off_twx = 0, off_twy = 0, off_twz = 0, off_psi = 0, off_acc = 0, off_w = 0, off_w0 = 0,
-         off_spec = 0, off_psf = 0, off_kern = 0, off_auto = 0, off_stage = 0, off_partials = 0,
+         off_spec = 0, off_psf = 0, off_kern = 0, off_auto = 0, off_partials = 0,
          off_scalars = 0, off_cmp = 0, total = 0;
   size_t psf_stride = 0, auto_stride = 0;   // elements (doubles) per view
   int sum_blocks = 0;
@@ -335,7 +335,6 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
   P.off_psf = take(P.psf_stride * sizeof(double) * P.V);
   P.off_kern = take(P.psf_stride * sizeof(double) * P.V);
   P.off_auto = take(kmode == MVD_KERNEL_COMPOUND ? P.auto_stride * sizeof(double) * P.V : 256);
-  P.off_stage = take(P.psf_stride * sizeof(float));
   P.sum_blocks = reduce_blocks();
   P.off_partials = take(sizeof(double) * 2 * (size_t)std::max(P.nctax, P.sum_blocks * kMaxZChunks));
   P.off_scalars = take(sizeof(double) * (size_t)(P.V + 8));
@@ -358,6 +357,7 @@ struct mvd_ctx {
   float eps = 1e-6f, psi_floor = 1e-6f, tikhonov = 0.f;
   cudaStream_t stream = nullptr;
   char* ws = nullptr;
+  char* psf_staging = nullptr;   // pinned, device-mapped host copy of the PSF taps; lives for the duration of mvd_create
   std::vector<const float*> views;
   std::vector<const float*> weights;   // empty or one per view (borrowed)
   std::vector<char> is_local;          // view-parallel contexts: which views this context owns (all by default)
@@ -378,7 +378,7 @@ struct mvd_ctx {
   int graph_stats_ncta = 0;          // CTAs of the update kernel that write the statistics partials (as captured)
   char err[512] = {0};
   int num_sms = 148;
-  int xt_blocks[5] = {0, 0, 0, 0, 0};   // resident CTAs per SM of the TMA-staged x pass, per mode
+  int xt_blocks[5][4] = {};          // resident CTAs per SM of the TMA-staged x pass, per (mode, compile-time flags)
   int flip = 0;                      // tile direction of the next x / y launch (alternates: L2 reuse)
   int use_flip = 1;
   int yt_blocks[2] = {0, 0};         // ... of the TMA-staged y pass (forward, inverse)
@@ -410,7 +410,6 @@ struct mvd_ctx {
   double* psf(int v) { return reinterpret_cast<double*>(ws + P.off_psf) + (size_t)v * P.psf_stride; }
   double* kern(int v) { return reinterpret_cast<double*>(ws + P.off_kern) + (size_t)v * P.psf_stride; }
   double* autoc(int v) { return reinterpret_cast<double*>(ws + P.off_auto) + (size_t)v * P.auto_stride; }
-  float* stage() { return reinterpret_cast<float*>(ws + P.off_stage); }
   double* partials() { return reinterpret_cast<double*>(ws + P.off_partials); }
   double* scalars() { return reinterpret_cast<double*>(ws + P.off_scalars); }   // [0..V) view sums, [V],[V+1] stats
 
@@ -614,12 +613,14 @@ mvd_status x_pass(mvd_ctx* c, const XArgs& a_in, int mode) {
     const float* real_src = mode == X_QUOT ? a.phi : (mode == X_ACCUM ? a.acc : a.psi);
     a.bulk_real = (P.N[0] % 4 == 0) && ((reinterpret_cast<size_t>(real_src) & 15) == 0) &&
                   ((reinterpret_cast<size_t>(a.wts) & 15) == 0);
-    if (c->xt_blocks[mode] == 0) {
-      c->xt_blocks[mode] = P.lx->xrow_tma_blocks_per_sm(mode, a.nthreads, P.lx->xrow_tma_smem(a.rows_per_cta, P.r[0], P.N[0], mode == X_UPDATE_W));
-      if (c->xt_blocks[mode] <= 0) { snprintf(c->err, sizeof(c->err), "x pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
+    const int flags = P.lx->xrow_tma_flags(a, mode) & 3;
+    int& bl = c->xt_blocks[mode][flags];
+    if (bl == 0) {
+      bl = P.lx->xrow_tma_blocks_per_sm(mode, flags, a.nthreads, P.lx->xrow_tma_smem(a.rows_per_cta, P.r[0], P.N[0], mode == X_UPDATE_W));
+      if (bl <= 0) { snprintf(c->err, sizeof(c->err), "x pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
     }
     const long long ntiles = (a.nrows + a.rows_per_cta - 1) / a.rows_per_cta;
-    a.grid = (int)std::min<long long>(std::min<long long>(ntiles, (long long)c->num_sms * c->xt_blocks[mode]), P.sum_blocks);
+    a.grid = (int)std::min<long long>(std::min<long long>(ntiles, (long long)c->num_sms * bl), P.sum_blocks);
     {
       ProfScope ps(c, cls[mode]);
       MVD_CK(P.lx->xrow_tma(a, mode, c->stream), "x pass (TMA)");
@@ -773,36 +774,42 @@ mvd_status build_spectrum(mvd_ctx* c, const double* kern, Dims3 K, float2* spec)
 // context per block shape, same PSFs), V * psf_stride doubles on the device; NULL -> compute them
 mvd_status precompute(mvd_ctx* c, const float* const* psfs_host, const double* shared_kern) {
   const Plan& P = c->P;
-  // twiddle tables, generated in double
+  // twiddle tables, generated on the device in double.  mvd_create issues NO host-to-device copy: a copy would
+  // queue on the copy engine behind the caller's (possibly still running) upload of the views and serialise the
+  // whole precompute with it (measured: 34 ms of H2D + 31 ms of precompute instead of max of the two)
   {
     const int M[3] = {P.Mx, P.My, P.Mz};
     float2* dst[3] = {c->twx(), c->twy(), c->twz()};
     for (int a = 0; a < 3; ++a) {
-      std::vector<float2> t(M[a]);
-      for (int j = 0; j < M[a]; ++j) {
-        const double ang = -2.0 * M_PI * (double)j / (double)M[a];
-        t[j] = make_float2((float)cos(ang), (float)sin(ang));
-      }
-      MVD_CK(cudaMemcpyAsync(dst[a], t.data(), sizeof(float2) * M[a], cudaMemcpyHostToDevice, c->stream), "twiddle upload");
-      MVD_CK(cudaStreamSynchronize(c->stream), "twiddle upload");
+      twiddle_kernel<<<(M[a] + 255) / 256, 256, 0, c->stream>>>(dst[a], M[a]);
+      MVD_CK(cudaGetLastError(), "twiddle_kernel");
+      ++c->launches;
     }
   }
-  // normalised PSFs in fp64 (eq. 4)
-  for (int v = 0; v < P.V; ++v) {
-    const Dims3 K = P.K[v];
-    const int n = K.x * K.y * K.z;
-    double hsum = 0.0;
-    for (int i = 0; i < n; ++i) {
-      const float t = psfs_host[v][i];
-      if (!(t >= 0.f) || !std::isfinite(t)) { snprintf(c->err, sizeof(c->err), "PSF %d has a negative or non-finite tap", v); return MVD_ERR_INVALID_ARG; }
-      hsum += t;
+  // normalised PSFs in fp64 (eq. 4): the taps are staged in pinned host memory that the device reads in place
+  {
+    size_t total = 0;
+    for (int v = 0; v < P.V; ++v) total += align_up((size_t)P.K[v].x * P.K[v].y * P.K[v].z * sizeof(float), 256);
+    MVD_CK(cudaHostAlloc(reinterpret_cast<void**>(&c->psf_staging), total, cudaHostAllocMapped), "pinned PSF staging");
+    char* dev_base = nullptr;
+    MVD_CK(cudaHostGetDevicePointer(reinterpret_cast<void**>(&dev_base), c->psf_staging, 0), "pinned PSF staging");
+    size_t off = 0;
+    for (int v = 0; v < P.V; ++v) {
+      const Dims3 K = P.K[v];
+      const int n = K.x * K.y * K.z;
+      double hsum = 0.0;
+      for (int i = 0; i < n; ++i) {
+        const float t = psfs_host[v][i];
+        if (!(t >= 0.f) || !std::isfinite(t)) { snprintf(c->err, sizeof(c->err), "PSF %d has a negative or non-finite tap", v); return MVD_ERR_INVALID_ARG; }
+        hsum += t;
+      }
+      if (!(hsum > 0.0)) { snprintf(c->err, sizeof(c->err), "PSF %d sums to zero", v); return MVD_ERR_INVALID_ARG; }
+      memcpy(c->psf_staging + off, psfs_host[v], sizeof(float) * n);
+      normalise_kernel<float><<<1, 1024, 0, c->stream>>>(reinterpret_cast<const float*>(dev_base + off), n, c->psf(v));
+      MVD_CK(cudaGetLastError(), "normalise_kernel");
+      ++c->launches;
+      off += align_up(sizeof(float) * n, 256);
     }
-    if (!(hsum > 0.0)) { snprintf(c->err, sizeof(c->err), "PSF %d sums to zero", v); return MVD_ERR_INVALID_ARG; }
-    MVD_CK(cudaMemcpyAsync(c->stage(), psfs_host[v], sizeof(float) * n, cudaMemcpyHostToDevice, c->stream), "PSF upload");
-    normalise_kernel<float><<<1, 1024, 0, c->stream>>>(c->stage(), n, c->psf(v));
-    MVD_CK(cudaGetLastError(), "normalise_kernel");
-    ++c->launches;
-    MVD_CK(cudaStreamSynchronize(c->stream), "PSF upload");   // the staging buffer is reused
   }
   // back-projectors K_v (O3)
   if (shared_kern) {
@@ -1017,6 +1024,11 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
     s = MVD_ERR_CUDA;
   if (s == MVD_OK) s = init_estimate(c, opt->psi0);
   if (s == MVD_OK && c->fail(cudaStreamSynchronize(c->stream), "mvd_create")) s = MVD_ERR_CUDA;
+  if (c->psf_staging) {
+    if (s != MVD_OK) cudaStreamSynchronize(c->stream);   // a kernel may still be reading the staged taps
+    cudaFreeHost(c->psf_staging);
+    c->psf_staging = nullptr;
+  }
   if (s != MVD_OK) {
     if (c->err[0]) fprintf(stderr, "mvd_create: %s\n", c->err);
     delete c;

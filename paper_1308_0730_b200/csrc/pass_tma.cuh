@@ -39,7 +39,11 @@ constexpr int kTmaTile = kTmaTileHost;
 constexpr int kXrowTmaThreads = 160;
 constexpr int xrow_min_blocks(int ab_max) { return ab_max <= 21 ? 4 : (ab_max <= 28 ? 3 : 2); }
 
-template <int A, int B, int MODE>
+// FLAGS (compile-time, so the common kernels carry no code for the rare paths): XF_TIK = Tikhonov-regularised
+// update (mvd.h, R14); XF_LAST = the last view of a combined iteration (root, psi update, forward transform)
+enum XFlags { XF_TIK = 1, XF_LAST = 2 };
+
+template <int A, int B, int MODE, int FLAGS>
 __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>::AB_MAX)) xrow_tma_kernel(const XArgs p) {
   using Cfg = PassCfg<A, B>;
   constexpr int M = Cfg::M, AP = Cfg::AP, BP = Cfg::BP;
@@ -47,9 +51,12 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
   static_assert(MODE == X_QUOT || MODE == X_UPDATE || MODE == X_UPDATE_W || MODE == X_ACCUM, "TMA-staged x pass: no X_LOAD");
   // X_ACCUM (combined variants): running product of the f_v in acc; the last view takes the root,
   // updates psi and transforms the new estimate.  acc is the staged real row (read for MID / LAST).
+  static_assert(MODE == X_ACCUM || !(FLAGS & XF_LAST), "XF_LAST belongs to X_ACCUM");
+  static_assert(MODE != X_QUOT && (MODE != X_ACCUM || (FLAGS & XF_LAST)) || !(FLAGS & XF_TIK), "XF_TIK belongs to the psi updates");
+  constexpr bool tik = (FLAGS & XF_TIK) != 0;
   const bool acc_read = MODE == X_ACCUM && (p.acc_mode == ACC_MID || p.acc_mode == ACC_LAST);
-  const bool acc_last = MODE == X_ACCUM && (p.acc_mode == ACC_LAST || p.acc_mode == ACC_ONLY);
-  const bool do_forward = MODE != X_ACCUM || acc_last;
+  constexpr bool acc_last = MODE == X_ACCUM && (FLAGS & XF_LAST) != 0;   // acc_mode is ACC_LAST or ACC_ONLY
+  constexpr bool do_forward = MODE != X_ACCUM || acc_last;
   const bool need_real = MODE != X_ACCUM || acc_read;          // real rows staged at all
   const bool real_bulk = need_real && p.bulk_real, real_plain = need_real && !p.bulk_real;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -188,7 +195,9 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
         } else if constexpr (MODE == X_UPDATE || MODE == X_UPDATE_W) {
           const float o = rrow[x];
           if (has_w) v = fmaf(wrow[x], v - 1.f, 1.f);                     // section 12: fraction w of the RL step
-          const float nw = fmaxf(tikhonov_update(o * v, p.tikhonov), p.psi_floor);   // eq. 109-112, R4, R14
+          float u = o * v;
+          if constexpr (tik) u = tikhonov_value(u, p.tikhonov);           // R14
+          const float nw = fmaxf(u, p.psi_floor);                         // eq. 109-112, R4
           prow[x] = nw;
           flux += nw;
           l1 += fabsf(nw - o);
@@ -196,13 +205,17 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
         } else {                                                          // X_ACCUM (eq. 70 / 104, R1)
           float f = p.literal_product ? v : fmaxf(v, 0.f);
           if (acc_read) f *= rrow[x];
-          if (!acc_last) {
+          if constexpr (!acc_last) {
             arow[x] = f;
             return 0.f;
           }
-          if (!p.literal_product && p.inv_nviews != 1.f) f = powf(f, p.inv_nviews);
+          // eq. 44: the |V|-th root as exp2(log2(f) / V) on the special-function unit (f is a product of V
+          // ratios near 1: the hardware log2 / exp2 keep the relative error at a few 1e-7)
+          if (!p.literal_product && p.inv_nviews != 1.f) f = __powf(f, p.inv_nviews);
           const float o = prow[x];
-          const float nw = fmaxf(tikhonov_update(o * f, p.tikhonov), p.psi_floor);
+          float u = o * f;
+          if constexpr (tik) u = tikhonov_value(u, p.tikhonov);           // R14
+          const float nw = fmaxf(u, p.psi_floor);
           prow[x] = nw;
           flux += nw;
           l1 += fabsf(nw - o);
@@ -538,10 +551,14 @@ struct LaunchTma {
   if (e != cudaSuccess) { fprintf(stderr, "smem attr failed %d x %d: %s\n", A, B, #k); return e; } \
   e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); \
   if (e != cudaSuccess) { fprintf(stderr, "carveout attr failed %d x %d: %s\n", A, B, #k); return e; }
-    MVD_SET((xrow_tma_kernel<A, B, X_QUOT>));
-    MVD_SET((xrow_tma_kernel<A, B, X_UPDATE>));
-    MVD_SET((xrow_tma_kernel<A, B, X_ACCUM>));
-    MVD_SET((xrow_tma_kernel<A, B, X_UPDATE_W>));
+    MVD_SET((xrow_tma_kernel<A, B, X_QUOT, 0>));
+    MVD_SET((xrow_tma_kernel<A, B, X_UPDATE, 0>));
+    MVD_SET((xrow_tma_kernel<A, B, X_UPDATE, XF_TIK>));
+    MVD_SET((xrow_tma_kernel<A, B, X_UPDATE_W, 0>));
+    MVD_SET((xrow_tma_kernel<A, B, X_UPDATE_W, XF_TIK>));
+    MVD_SET((xrow_tma_kernel<A, B, X_ACCUM, 0>));
+    MVD_SET((xrow_tma_kernel<A, B, X_ACCUM, XF_LAST>));
+    MVD_SET((xrow_tma_kernel<A, B, X_ACCUM, XF_LAST | XF_TIK>));
     MVD_SET((strided_tma_kernel<A, B, -1>));
     MVD_SET((strided_tma_kernel<A, B, 1>));
     MVD_SET((zconv_tma_kernel<A, B>));
@@ -549,16 +566,31 @@ struct LaunchTma {
     return cudaSuccess;
   }
 
-  static int xrow_blocks_per_sm(int mode, int nthreads, size_t smem) {
+  // the kernel of (mode, flags); flags: XF_TIK for a regularised update, XF_LAST for the last view of X_ACCUM
+  using XKernel = void (*)(const XArgs);
+  static XKernel xrow_kernel_of(int mode, int flags) {
+    const bool t = (flags & XF_TIK) != 0;
+    switch (mode) {
+      case X_QUOT: return xrow_tma_kernel<A, B, X_QUOT, 0>;
+      case X_UPDATE: return t ? xrow_tma_kernel<A, B, X_UPDATE, XF_TIK> : xrow_tma_kernel<A, B, X_UPDATE, 0>;
+      case X_UPDATE_W: return t ? xrow_tma_kernel<A, B, X_UPDATE_W, XF_TIK> : xrow_tma_kernel<A, B, X_UPDATE_W, 0>;
+      case X_ACCUM:
+        if (!(flags & XF_LAST)) return xrow_tma_kernel<A, B, X_ACCUM, 0>;
+        return t ? xrow_tma_kernel<A, B, X_ACCUM, XF_LAST | XF_TIK> : xrow_tma_kernel<A, B, X_ACCUM, XF_LAST>;
+      default: return nullptr;
+    }
+  }
+  static int xrow_flags(const XArgs& a, int mode) {
+    const bool last = mode == X_ACCUM && (a.acc_mode == ACC_LAST || a.acc_mode == ACC_ONLY);
+    const bool upd = mode == X_UPDATE || mode == X_UPDATE_W || last;
+    return (last ? XF_LAST : 0) | ((upd && a.tikhonov > 0.f) ? XF_TIK : 0);
+  }
+
+  static int xrow_blocks_per_sm(int mode, int flags, int nthreads, size_t smem) {
     int n = 0;
-    cudaError_t e = mode == X_QUOT
-        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_QUOT>, nthreads, smem)
-        : mode == X_UPDATE
-        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_UPDATE>, nthreads, smem)
-        : mode == X_ACCUM
-        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_ACCUM>, nthreads, smem)
-        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, xrow_tma_kernel<A, B, X_UPDATE_W>, nthreads, smem);
-    return e == cudaSuccess ? n : 0;
+    XKernel k = xrow_kernel_of(mode, flags);
+    if (!k) return 0;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k, nthreads, smem) == cudaSuccess ? n : 0;
   }
 
   static size_t strided_smem(int T, int boxr, int nbox, int nst) {
@@ -595,13 +627,12 @@ struct LaunchTma {
   static cudaError_t xrow(const XArgs& a, int mode, cudaStream_t s) {
     if (a.grid <= 0) return cudaSuccess;
     const size_t smem = xrow_smem(a.rows_per_cta, a.rx, a.nx, mode == X_UPDATE_W);
-    if (mode == X_QUOT) xrow_tma_kernel<A, B, X_QUOT><<<a.grid, a.nthreads, smem, s>>>(a);
-    else if (mode == X_UPDATE) xrow_tma_kernel<A, B, X_UPDATE><<<a.grid, a.nthreads, smem, s>>>(a);
-    else if (mode == X_ACCUM) xrow_tma_kernel<A, B, X_ACCUM><<<a.grid, a.nthreads, smem, s>>>(a);
-    else if (mode == X_UPDATE_W) xrow_tma_kernel<A, B, X_UPDATE_W><<<a.grid, a.nthreads, smem, s>>>(a);
-    else return cudaErrorInvalidValue;
+    XKernel k = xrow_kernel_of(mode, xrow_flags(a, mode));
+    if (!k) return cudaErrorInvalidValue;
+    k<<<a.grid, a.nthreads, smem, s>>>(a);
     return cudaGetLastError();
   }
+  static int xrow_flags_of(const XArgs& a, int mode) { return xrow_flags(a, mode); }
 };
 
 }  // namespace mvd
