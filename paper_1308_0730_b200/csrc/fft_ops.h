@@ -32,6 +32,7 @@ struct StridedTmaArgs {
   int n_out;               // pencil outputs >= n_out are not stored
   int reverse;             // walk the tiles last to first (reads what the previous pass wrote last: L2 hits)
   int nst;                 // shared-memory stages of the tile: 1 or 2
+  int cluster;             // > 1: launched as clusters of this many CTAs that pace their prefetches together
 };
 
 // ---- TMA-staged fused z pass: input tile and spectrum tile by tensor copies --------------------
@@ -47,6 +48,7 @@ struct ZconvTmaArgs {
   long long plane;         // elements between z planes of `out`
   int nz;                  // planes written
   int nst_in;              // shared-memory stages of the input tile: 1 or 2
+  int cluster;             // > 1: clusters of this many CTAs pace their prefetches together
 };
 
 // ---- strided pencil FFT (y pass, plain z pass): pencils along a strided axis, tiles of T

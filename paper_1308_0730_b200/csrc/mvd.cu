@@ -365,6 +365,8 @@ struct mvd_ctx {
   float psi0_value = 0.f;
   bool w_valid = false;        // the work buffer holds the x-forward transform of the current psi
                                // (z-chunked schedule: the x- and y-forward transform)
+  int ycluster = 1;            // CTAs per cluster of the TMA-staged y pass (1 = plain launch)
+  int zcluster = 1;            // ... of the TMA-staged z pass
   int zchunk = 0;              // > 0: the plane-local passes (y-inverse, x pass, y-forward) run chunk by chunk of this
                                // many z planes, so a chunk of the work buffer stays in L2 between them
   bool broken = false;
@@ -496,6 +498,11 @@ mvd_status y_pass_tma(mvd_ctx* c, float2* buf, int dir, int nz_planes, int xt0, 
   if (bl == 0) bl = P.ly->strided_tma_blocks_per_sm(dir, a.nthreads, P.ly->strided_tma_smem(a.T, a.boxr, a.nbox, a.nst));
   if (bl <= 0) { snprintf(c->err, sizeof(c->err), "y pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
   a.grid = (int)std::min<long long>((long long)n_xt * nz_planes, (long long)c->num_sms * bl);
+  a.cluster = c->ycluster;
+  if (a.cluster > 1) {
+    a.grid = a.grid / a.cluster * a.cluster;
+    if (a.grid == 0) { a.grid = 1; a.cluster = 1; }
+  }
   {
     ProfScope ps(c, dir < 0 ? MVD_K_Y_FWD : MVD_K_Y_INV);
     MVD_CK(P.ly->strided_tma(a, dir, c->stream), "y pass (TMA)");
@@ -520,6 +527,11 @@ mvd_status z_conv_tma(mvd_ctx* c, const float2* in, float2* out, const float2* s
   if (c->zt_blocks == 0) c->zt_blocks = P.lz->zconv_tma_blocks_per_sm(a.nthreads, P.lz->zconv_tma_smem(a.T, a.boxr, a.nbox, a.nst_in));
   if (c->zt_blocks <= 0) { snprintf(c->err, sizeof(c->err), "z pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
   a.grid = (int)std::min<long long>((long long)n_xt * ((P.My + 1) / 2), (long long)c->num_sms * c->zt_blocks);
+  a.cluster = c->zcluster;
+  if (a.cluster > 1) {
+    a.grid = a.grid / a.cluster * a.cluster;
+    if (a.grid == 0) { a.grid = 1; a.cluster = 1; }
+  }
   {
     ProfScope ps(c, MVD_K_Z_CONV);
     MVD_CK(P.lz->zconv_tma(a, c->stream), "z convolution pass (TMA)");
@@ -986,6 +998,8 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
   c->ws = reinterpret_cast<char*>(opt->workspace);
   c->use_graph = opt->use_graph;
   c->use_flip = env_int("MVD_FLIP", 1);
+  c->ycluster = std::min(8, std::max(1, env_int("MVD_YCLUSTER", 1)));
+  c->zcluster = std::min(8, std::max(1, env_int("MVD_ZCLUSTER", 1)));
   c->zchunk = std::max(0, env_int("MVD_ZCHUNK", 0));
   if (c->zchunk > 0) c->zchunk = std::max(c->zchunk, (c->P.N[2] + kMaxZChunks - 1) / kMaxZChunks);
   if (c->use_graph && !c->stream) {   // the legacy default stream cannot be captured

@@ -341,8 +341,15 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
 
   if (tid == 0 && (int)blockIdx.x < ntiles) issue((int)blockIdx.x, 0);
 
+  // p.cluster > 1: the CTAs of a cluster take adjacent x tiles and meet at a cluster barrier before every prefetch,
+  // so the copies of one memory row (cluster * T contiguous elements) are issued together
+  const int rounds = p.cluster > 1 ? (ntiles + (int)gridDim.x - 1) / (int)gridDim.x : 0;
   int it = 0;
-  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+  for (int tile = blockIdx.x; p.cluster > 1 ? it < rounds : tile < ntiles; tile += gridDim.x, ++it) {
+    if (p.cluster > 1) {
+      cluster_arrive_wait();
+      if (tile >= ntiles) continue;
+    }
     const int s = nst == 2 ? (it & 1) : 0;
     float2* sm = buf + (size_t)s * NR * T;
     const bool more = tile + (int)gridDim.x < ntiles;
@@ -450,8 +457,13 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
     issue_spec((int)blockIdx.x);
   }
 
+  const int rounds = p.cluster > 1 ? (ntiles + (int)gridDim.x - 1) / (int)gridDim.x : 0;   // see strided_tma_kernel
   int it = 0;
-  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+  for (int tile = blockIdx.x; p.cluster > 1 ? it < rounds : tile < ntiles; tile += gridDim.x, ++it) {
+    if (p.cluster > 1) {
+      cluster_arrive_wait();
+      if (tile >= ntiles) continue;
+    }
     const int s = nst == 2 ? (it & 1) : 0;
     float2* sm = buf + (size_t)s * NR * T;
     const float2* sp = sbuf;
@@ -614,13 +626,45 @@ struct LaunchTma {
   static cudaError_t strided(const StridedTmaArgs& a, int dir, cudaStream_t s) {
     if (a.grid <= 0) return cudaSuccess;
     const size_t smem = strided_smem(a.T, a.boxr, a.nbox, a.nst);
+    if (a.cluster > 1) {
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)a.grid);
+      cfg.blockDim = dim3((unsigned)a.nthreads);
+      cfg.dynamicSmemBytes = smem;
+      cfg.stream = s;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = (unsigned)a.cluster;
+      at[0].val.clusterDim.y = 1;
+      at[0].val.clusterDim.z = 1;
+      cfg.attrs = at;
+      cfg.numAttrs = 1;
+      return dir < 0 ? cudaLaunchKernelEx(&cfg, strided_tma_kernel<A, B, -1>, a)
+                     : cudaLaunchKernelEx(&cfg, strided_tma_kernel<A, B, 1>, a);
+    }
     if (dir < 0) strided_tma_kernel<A, B, -1><<<a.grid, a.nthreads, smem, s>>>(a);
     else strided_tma_kernel<A, B, 1><<<a.grid, a.nthreads, smem, s>>>(a);
     return cudaGetLastError();
   }
   static cudaError_t zconv(const ZconvTmaArgs& a, cudaStream_t s) {
     if (a.grid <= 0) return cudaSuccess;
-    zconv_tma_kernel<A, B><<<a.grid, a.nthreads, zconv_smem(a.T, a.boxr, a.nbox, a.nst_in), s>>>(a);
+    const size_t smem = zconv_smem(a.T, a.boxr, a.nbox, a.nst_in);
+    if (a.cluster > 1) {
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)a.grid);
+      cfg.blockDim = dim3((unsigned)a.nthreads);
+      cfg.dynamicSmemBytes = smem;
+      cfg.stream = s;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = (unsigned)a.cluster;
+      at[0].val.clusterDim.y = 1;
+      at[0].val.clusterDim.z = 1;
+      cfg.attrs = at;
+      cfg.numAttrs = 1;
+      return cudaLaunchKernelEx(&cfg, zconv_tma_kernel<A, B>, a);
+    }
+    zconv_tma_kernel<A, B><<<a.grid, a.nthreads, smem, s>>>(a);
     return cudaGetLastError();
   }
 
