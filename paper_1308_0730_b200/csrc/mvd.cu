@@ -365,6 +365,7 @@ struct mvd_ctx {
   float psi0_value = 0.f;
   bool w_valid = false;        // the work buffer holds the x-forward transform of the current psi
                                // (z-chunked schedule: the x- and y-forward transform)
+  int y_tensor_store = 0;      // y pass: results leave by tensor copies from the staged tile instead of per-thread stores
   int ycluster = 1;            // CTAs per cluster of the TMA-staged y pass (1 = plain launch)
   int zcluster = 1;            // ... of the TMA-staged z pass
   int zchunk = 0;              // > 0: the plane-local passes (y-inverse, x pass, y-forward) run chunk by chunk of this
@@ -488,6 +489,12 @@ mvd_status y_pass_tma(mvd_ctx* c, float2* buf, int dir, int nz_planes, int xt0, 
     return MVD_ERR_CUDA;
   }
   a.out = buf; a.tw = c->twy();
+  a.tensor_store = c->y_tensor_store;
+  if (a.tensor_store && !make_map3(&a.out_map, buf, P.Mx, dir < 0 ? P.My : P.N[1], nz_planes, P.Mx, P.plane, P.Tyt, P.ybox, 1)) {
+    snprintf(c->err, sizeof(c->err), "y pass: cuTensorMapEncodeTiled failed");
+    c->broken = true;
+    return MVD_ERR_CUDA;
+  }
   a.T = P.Tyt; a.nthreads = P.ntyt; a.boxr = P.ybox; a.nbox = P.ynbox;
   a.xt0 = xt0; a.n_xt = n_xt; a.nst = P.ynst;
   a.line_len = P.Mx; a.n_outer = nz_planes;
@@ -998,6 +1005,7 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
   c->ws = reinterpret_cast<char*>(opt->workspace);
   c->use_graph = opt->use_graph;
   c->use_flip = env_int("MVD_FLIP", 1);
+  c->y_tensor_store = env_int("MVD_YTSTORE", 0) ? 1 : 0;
   c->ycluster = std::min(8, std::max(1, env_int("MVD_YCLUSTER", 1)));
   c->zcluster = std::min(8, std::max(1, env_int("MVD_ZCLUSTER", 1)));
   c->zchunk = std::max(0, env_int("MVD_ZCHUNK", 0));

@@ -307,8 +307,19 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
 //   stage 1: item (n2, x) owns rows n1*B + n2 -> A-point FFT, twiddle -> rows k1*B + n2
 //   stage 2: item (k1, x) owns rows k1*B + n2 -> B-point FFT -> global rows k1 + A*k2 (< n_out)
 // =========================================================================================
-template <int A, int B, int DIR>
-__global__ void __launch_bounds__(PassCfg<A, B>::MAX_THREADS)
+// TS: the stage-2 results are written back into the staged tile (after every item has read its inputs) and leave
+// by tensor copies (SASS UTMASTG) instead of per-thread stores; needs a single round of stage-2 items per tile.
+// threads the planner gives the y pass of this length (one round of items per stage when they fit)
+template <int A, int B>
+constexpr int strided_tma_threads() {
+  constexpr int items = strided_tma_tile(A * B) * PassCfg<A, B>::AB_MAX;
+  constexpr int rounds = (items + PassCfg<A, B>::MAX_THREADS - 1) / PassCfg<A, B>::MAX_THREADS;
+  constexpr int t = ((items + rounds - 1) / rounds + 31) / 32 * 32;
+  return t < PassCfg<A, B>::MAX_THREADS ? t : PassCfg<A, B>::MAX_THREADS;
+}
+
+template <int A, int B, int DIR, bool TS>
+__global__ void __launch_bounds__(TS ? strided_tma_threads<A, B>() : PassCfg<A, B>::MAX_THREADS, TS ? 2 : 0)
 strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
   constexpr int M = A * B;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -353,7 +364,9 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
     const int s = nst == 2 ? (it & 1) : 0;
     float2* sm = buf + (size_t)s * NR * T;
     const bool more = tile + (int)gridDim.x < ntiles;
-    if (tid == 0 && more && nst == 2) issue(tile + (int)gridDim.x, s ^ 1);
+    // tensor stores: the other stage is still being read by the previous tile's store; its refill waits until
+    // after stage 1 of this tile
+    if (tid == 0 && more && nst == 2 && !TS) issue(tile + (int)gridDim.x, s ^ 1);
     const int rtile = p.reverse ? ntiles - 1 - tile : tile;
     const int outer = rtile / p.n_xt;
     const int x0 = (p.xt0 + (rtile - outer * p.n_xt)) * T;
@@ -378,28 +391,68 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
       });
     }
     __syncthreads();
-    float2* out = p.out + (long long)outer * p.out_outer_stride + x0;
-    for (int j = tid; j < T * A; j += blockDim.x) {
+    if constexpr (TS) {
+      if (tid == 0 && more && nst == 2) {
+        bulk_wait_read0();                       // the previous tile's store has read the other stage
+        issue(tile + (int)gridDim.x, s ^ 1);
+      }
+      const int j = tid;                         // one round: T * A <= blockDim.x (checked by the host)
       const int k1 = j / T;
       const int x = j - k1 * T;
+      const bool act = j < T * A;
       float2 u[B];
-      static_for<0, B>([&](auto n2_) {
-        constexpr int n2 = decltype(n2_)::value;
-        u[n2] = sm[(k1 * B + n2) * T + x];
-      });
-      FftReg<B, DIR>::run(u);
-      if (x < xvalid) {
-        float2* o = out + (long long)k1 * p.out_pstride + x;
+      if (act) {
+        static_for<0, B>([&](auto n2_) {
+          constexpr int n2 = decltype(n2_)::value;
+          u[n2] = sm[(k1 * B + n2) * T + x];
+        });
+        FftReg<B, DIR>::run(u);
+      }
+      __syncthreads();                           // every input of the tile has been read
+      if (act) {
         static_for<0, B>([&](auto k2_) {
           constexpr int k2 = decltype(k2_)::value;
-          if (k1 + A * k2 < p.n_out) o[(long long)(A * k2) * p.out_pstride] = u[k2];
+          sm[(k1 + A * k2) * T + x] = u[k2];
         });
       }
+      fence_proxy_async();                       // generic-proxy stores -> visible to the copy engine
+      __syncthreads();
+      if (tid == 0) {
+        for (int b = 0; b < p.nbox; ++b)
+          if (b * p.boxr < p.n_out) tma_store_3d(&p.out_map, sm + (size_t)(b * p.boxr) * T, x0, b * p.boxr, outer);
+        bulk_commit();
+        if (more && nst == 1) {
+          bulk_wait_read0();
+          issue(tile + (int)gridDim.x, 0);
+        }
+      }
+    } else {
+      float2* out = p.out + (long long)outer * p.out_outer_stride + x0;
+      for (int j = tid; j < T * A; j += blockDim.x) {
+        const int k1 = j / T;
+        const int x = j - k1 * T;
+        float2 u[B];
+        static_for<0, B>([&](auto n2_) {
+          constexpr int n2 = decltype(n2_)::value;
+          u[n2] = sm[(k1 * B + n2) * T + x];
+        });
+        FftReg<B, DIR>::run(u);
+        if (x < xvalid) {
+          float2* o = out + (long long)k1 * p.out_pstride + x;
+          static_for<0, B>([&](auto k2_) {
+            constexpr int k2 = decltype(k2_)::value;
+            if (k1 + A * k2 < p.n_out) o[(long long)(A * k2) * p.out_pstride] = u[k2];
+          });
+        }
+      }
+      // the tile was transformed in place by ordinary stores; the copy engine (async proxy) refills it
+      fence_proxy_async();
+      __syncthreads();   // every read of this tile is done
+      if (tid == 0 && more && nst == 1) issue(tile + (int)gridDim.x, 0);   // one stage: refill it now
     }
-    // the tile was transformed in place by ordinary stores; the copy engine (async proxy) refills it
-    fence_proxy_async();
-    __syncthreads();   // every read of this tile is done
-    if (tid == 0 && more && nst == 1) issue(tile + (int)gridDim.x, 0);   // one stage: refill it now
+  }
+  if constexpr (TS) {
+    if (tid == 0) bulk_wait_read0();             // shared memory must outlive the last store's reads
   }
 }
 
@@ -571,8 +624,10 @@ struct LaunchTma {
     MVD_SET((xrow_tma_kernel<A, B, X_ACCUM, 0>));
     MVD_SET((xrow_tma_kernel<A, B, X_ACCUM, XF_LAST>));
     MVD_SET((xrow_tma_kernel<A, B, X_ACCUM, XF_LAST | XF_TIK>));
-    MVD_SET((strided_tma_kernel<A, B, -1>));
-    MVD_SET((strided_tma_kernel<A, B, 1>));
+    MVD_SET((strided_tma_kernel<A, B, -1, false>));
+    MVD_SET((strided_tma_kernel<A, B, 1, false>));
+    MVD_SET((strided_tma_kernel<A, B, -1, true>));
+    MVD_SET((strided_tma_kernel<A, B, 1, true>));
     MVD_SET((zconv_tma_kernel<A, B>));
 #undef MVD_SET
     return cudaSuccess;
@@ -614,8 +669,8 @@ struct LaunchTma {
   static int strided_blocks_per_sm(int dir, int nthreads, size_t smem) {
     int n = 0;
     cudaError_t e = dir < 0
-        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, strided_tma_kernel<A, B, -1>, nthreads, smem)
-        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, strided_tma_kernel<A, B, 1>, nthreads, smem);
+        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, strided_tma_kernel<A, B, -1, false>, nthreads, smem)
+        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, strided_tma_kernel<A, B, 1, false>, nthreads, smem);
     return e == cudaSuccess ? n : 0;
   }
   static int zconv_blocks_per_sm(int nthreads, size_t smem) {
@@ -626,25 +681,23 @@ struct LaunchTma {
   static cudaError_t strided(const StridedTmaArgs& a, int dir, cudaStream_t s) {
     if (a.grid <= 0) return cudaSuccess;
     const size_t smem = strided_smem(a.T, a.boxr, a.nbox, a.nst);
-    if (a.cluster > 1) {
-      cudaLaunchConfig_t cfg = {};
-      cfg.gridDim = dim3((unsigned)a.grid);
-      cfg.blockDim = dim3((unsigned)a.nthreads);
-      cfg.dynamicSmemBytes = smem;
-      cfg.stream = s;
-      cudaLaunchAttribute at[1];
-      at[0].id = cudaLaunchAttributeClusterDimension;
-      at[0].val.clusterDim.x = (unsigned)a.cluster;
-      at[0].val.clusterDim.y = 1;
-      at[0].val.clusterDim.z = 1;
-      cfg.attrs = at;
-      cfg.numAttrs = 1;
-      return dir < 0 ? cudaLaunchKernelEx(&cfg, strided_tma_kernel<A, B, -1>, a)
-                     : cudaLaunchKernelEx(&cfg, strided_tma_kernel<A, B, 1>, a);
-    }
-    if (dir < 0) strided_tma_kernel<A, B, -1><<<a.grid, a.nthreads, smem, s>>>(a);
-    else strided_tma_kernel<A, B, 1><<<a.grid, a.nthreads, smem, s>>>(a);
-    return cudaGetLastError();
+    using K = void (*)(const StridedTmaArgs);
+    const bool ts = a.tensor_store && a.T * A <= a.nthreads;
+    K k = dir < 0 ? (ts ? (K)strided_tma_kernel<A, B, -1, true> : (K)strided_tma_kernel<A, B, -1, false>)
+                  : (ts ? (K)strided_tma_kernel<A, B, 1, true> : (K)strided_tma_kernel<A, B, 1, false>);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)a.grid);
+    cfg.blockDim = dim3((unsigned)a.nthreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)std::max(1, a.cluster);
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = a.cluster > 1 ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, k, a);
   }
   static cudaError_t zconv(const ZconvTmaArgs& a, cudaStream_t s) {
     if (a.grid <= 0) return cudaSuccess;
