@@ -24,7 +24,8 @@
  * Memory conventions
  *   - Volumes are fp32, x fastest: element (x,y,z) at [(z*Ny + y)*Nx + x].  dims = {Nx,Ny,Nz}.
  *   - `views` are DEVICE pointers; they are BORROWED (read-only, never copied) and must stay valid
- *     and unchanged until mvd_destroy.
+ *     until mvd_destroy, and unchanged while a call that reads them may be in flight (mvd_restart is
+ *     the call that accepts new contents).
  *   - `psfs` are HOST pointers, x fastest, dims psf_dims[v] = {Kx,Ky,Kz}, all odd (K may exceed N),
  *     values >= 0 with a positive sum (eq. 4).  They are copied during mvd_create.
  *   - ALL device memory the library uses is the caller's `workspace` (device pointer, at least
@@ -171,6 +172,15 @@ MVD_API mvd_status mvd_get_estimate(mvd_ctx* ctx, float* dst, int dst_is_device)
 
 /* Replaces the estimate (device pointer, N voxels); resume / fixed-point tests. */
 MVD_API mvd_status mvd_set_estimate(mvd_ctx* ctx, const float* src_device);
+
+/* Starts over on NEW CONTENTS of the same view buffers: the next time-point of a time-lapse acquired with the same
+ * PSFs (series of hundreds of time-points), so that the PSF precompute and the spectra of
+ * mvd_create are paid once per series.  The caller overwrites the borrowed view buffers (same pointers) after every
+ * earlier call on this context has completed, then calls mvd_restart: the stream waits for `views_ready` (optional
+ * cudaEvent_t recorded after the caller's copy, NULL = already there), the estimate is re-initialised exactly as
+ * mvd_create does (psi0 / psi0_value of the options, else the mean of the views), the iteration count and the
+ * statistics are reset.  Asynchronous on the stream. */
+MVD_API mvd_status mvd_restart(mvd_ctx* ctx, void* views_ready);
 
 /* Statistics of the LAST psi update: flux = sum psi_new, l1_change = sum |psi_new - psi_old|
  * (the reductions the paper's quality curves use, L127).  Synchronises.  Any pointer may be NULL. */

@@ -22,7 +22,7 @@ KERNEL_MODES = {"auto": 0, "plain": 1, "compound": 2, "opt1": 3, "opt2": 4}
 # every symbol include/mvd.h declares (tests check that the library exports them all)
 SYMBOLS = (
     "mvd_options_init", "mvd_workspace_size", "mvd_plan_dims", "mvd_create", "mvd_iterate",
-    "mvd_get_estimate", "mvd_set_estimate", "mvd_get_stats", "mvd_get_back_projector", "mvd_convolve",
+    "mvd_get_estimate", "mvd_set_estimate", "mvd_restart", "mvd_get_stats", "mvd_get_back_projector", "mvd_convolve",
     "mvd_launch_count", "mvd_profile", "mvd_profile_read", "mvd_kernel_class_name", "mvd_blocked_workspace_size", "mvd_deconvolve_blocked", "mvd_destroy",
     "mvd_status_string", "mvd_last_error",
     "mvd_compare", "mvd_partial_product", "mvd_get_product", "mvd_apply_product", "mvd_reduce_scratch_bytes", "mvd_reduce_sum",
@@ -86,6 +86,8 @@ def load_library():
     lib.mvd_get_estimate.restype = C.c_int
     lib.mvd_set_estimate.argtypes = [vp, vp]
     lib.mvd_set_estimate.restype = C.c_int
+    lib.mvd_restart.argtypes = [vp, vp]
+    lib.mvd_restart.restype = C.c_int
     lib.mvd_get_stats.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), ip]
     lib.mvd_get_stats.restype = C.c_int
     lib.mvd_get_back_projector.argtypes = [vp, C.c_int, vp]
@@ -326,6 +328,13 @@ class Deconvolver:
         self.stream.wait_stream(self._torch.cuda.current_stream(self.device))
         _check(self._lib.mvd_set_estimate(self._ctx, t.data_ptr()), self._ctx, "mvd_set_estimate")
         self.stream.synchronize()
+
+    def restart(self, views_ready=None):
+        """mvd_restart: the view buffers hold a new time-point (same PSFs); `views_ready` is a torch.cuda.Event
+        recorded after the caller's copy into them."""
+        ev = views_ready.cuda_event if views_ready is not None else None
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.mvd_restart(self._ctx, ev), self._ctx, "mvd_restart")
 
     def get_stats(self):
         f, l, it = C.c_double(), C.c_double(), C.c_int()

@@ -363,6 +363,7 @@ struct mvd_ctx {
   std::vector<char> is_local;          // view-parallel contexts: which views this context owns (all by default)
   bool partial = false;
   float psi0_value = 0.f;
+  const float* psi0_ptr = nullptr;     // options.psi0 (borrowed), for mvd_restart
   bool w_valid = false;        // the work buffer holds the x-forward transform of the current psi
                                // (z-chunked schedule: the x- and y-forward transform)
   int y_tensor_store = 0;      // y pass: results leave by tensor copies from the staged tile instead of per-thread stores
@@ -1044,6 +1045,7 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
   if (s == MVD_OK && opt->views_ready &&
       c->fail(cudaStreamWaitEvent(c->stream, reinterpret_cast<cudaEvent_t>(opt->views_ready), 0), "views_ready"))
     s = MVD_ERR_CUDA;
+  c->psi0_ptr = opt->psi0;
   if (s == MVD_OK) s = init_estimate(c, opt->psi0);
   if (s == MVD_OK && c->fail(cudaStreamSynchronize(c->stream), "mvd_create")) s = MVD_ERR_CUDA;
   if (c->psf_staging) {
@@ -1212,6 +1214,15 @@ mvd_status mvd_set_estimate(mvd_ctx* c, const float* src_device) {
   MVD_CK(cudaMemcpyAsync(c->psi(), src_device, sizeof(float) * (size_t)c->P.nvox, cudaMemcpyDeviceToDevice, c->stream), "estimate copy");
   c->w_valid = false;
   c->stats_valid = false;
+  return MVD_OK;
+}
+
+mvd_status mvd_restart(mvd_ctx* c, void* views_ready) {
+  if (!c) return MVD_ERR_INVALID_ARG;
+  if (c->broken) return MVD_ERR_STATE;
+  if (views_ready) MVD_CK(cudaStreamWaitEvent(c->stream, reinterpret_cast<cudaEvent_t>(views_ready), 0), "views_ready");
+  MVD_TRY(init_estimate(c, c->psi0_ptr));
+  c->iters = 0;
   return MVD_OK;
 }
 

@@ -277,6 +277,40 @@ def test_stats_after_set_estimate_graph_equals_plain_and_oracle(mvd, tiny, varia
     assert got[True][0]["l1_change"] == pytest.approx(o.l1_change, rel=2e-3)
 
 
+def test_restart_on_new_view_contents_equals_a_fresh_context(mvd, tiny):
+    """mvd_restart (time-lapse, L64 / L242): new contents in the same view buffers, same PSFs: bit-identical to a
+    context created on those contents, with plain launches and under graph replay; the oracle agrees."""
+    import torch
+    second = mvd_synth.make_tiny_asymmetric(seed_stream=3)        # another "time-point": other data ...
+    second_views = [v.copy() for v in second.views]
+    for use_graph in (False, True):
+        torch.cuda.synchronize()
+        kw = {"use_graph": True, "stream": torch.cuda.Stream()} if use_graph else {}
+        bufs = to_dev(tiny.views)
+        d = mvd.Deconvolver(bufs, tiny.psfs, variant="osem", **kw)
+        d.iterate(3)
+        first = d.get_estimate_host()
+        copy_stream = torch.cuda.Stream()
+        with torch.cuda.stream(copy_stream):
+            for b, v in zip(bufs, second_views):
+                b.copy_(torch.from_numpy(v), non_blocking=True)
+            ready = torch.cuda.Event()
+            ready.record(copy_stream)
+        d.restart(ready)
+        assert d.get_stats()["iterations_done"] == 0
+        d.iterate(3)
+        again = d.get_estimate_host()
+        st = d.get_stats()
+        d.close()
+        fresh, fst = gpu_checkpoints(mvd, mvd_synth.Problem(0, tiny.dims, tiny.psf_dims, tiny.gt, tiny.psfs, second_views, 3, ()),
+                                     "osem", "auto", (3,), **({"use_graph": True} if use_graph else {}))
+        assert np.array_equal(again, fresh[3]) and not np.array_equal(again, first)
+        assert st == fst
+    o = O.Oracle(second_views, tiny.psfs, "osem")                  # ... with the first time-point's PSFs
+    o.iterate(3)
+    check(again, o.psi, 3, "restart")
+
+
 def test_eps_and_floor_clamps(mvd, tiny):
     """R4: zero-valued data drive psi to the floor on both sides identically."""
     views = [v.copy() for v in tiny.views]
