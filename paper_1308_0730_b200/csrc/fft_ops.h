@@ -46,6 +46,7 @@ struct ZconvTmaArgs {
   int T, nthreads, grid;
   int boxr, nbox;
   int xt0, n_xt;           // x tiles [xt0, xt0 + n_xt) of every row
+  int tx;                  // contiguous x per tile: 8 (two rows y per tile) or 16 (one row)
   int mx, my;              // row length and rows per plane
   long long plane;         // elements between z planes of `out`
   int nz;                  // planes written
@@ -115,6 +116,7 @@ struct XArgs {
   float tikhonov;          // lambda of the Tikhonov-regularised update (0 = off), see mvd.h
   int acc_mode;            // AccMode
   int literal_product;
+  int root_each;           // X_ACCUM: every factor takes the |V|-th root before entering the product (many views)
   int complex_in;          // X_LOAD: rows of `in` are complex and transformed in full
   // TMA-staged variant (pass_tma.cuh)
   int real_stride;         // floats between real rows in shared memory

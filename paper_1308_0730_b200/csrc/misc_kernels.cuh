@@ -253,7 +253,7 @@ __global__ void __launch_bounds__(256) apply_product_kernel(float* __restrict__ 
   const long long stride = (long long)gridDim.x * blockDim.x;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
     float f = acc[i];
-    if (!literal && inv_nviews != 1.f) f = powf(f, inv_nviews);
+    if (!literal && inv_nviews != 1.f) f = __powf(f, inv_nviews);   // literal: also set when the factors were rooted one by one
     const float o = psi[i];
     float u = o * f;
     if (tikhonov > 0.f) {                                      // mvd.h, R14 (same arithmetic as tikhonov_value of the x pass)

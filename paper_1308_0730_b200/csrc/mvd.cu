@@ -150,6 +150,9 @@ static int sm_count() {
 // grid of the grid-stride reduction / fill kernels: 8 CTAs of 256 threads per SM
 static int reduce_blocks() { return 8 * sm_count(); }
 
+// combined variants: the running product of the f_v is kept in fp32; beyond this many views every factor takes the
+// |V|-th root before it enters the product (same value, no overflow or underflow for any V the ABI accepts)
+constexpr int kRootEachViews = 16;
 constexpr int kMaxZChunks = 64;   // z-chunked schedule: at most this many chunks (one statistics slot each)
 
 static int env_int(const char* name, int dflt) {
@@ -369,6 +372,7 @@ struct mvd_ctx {
   int y_tensor_store = 0;      // y pass: results leave by tensor copies from the staged tile instead of per-thread stores
   int ycluster = 1;            // CTAs per cluster of the TMA-staged y pass (1 = plain launch)
   int zcluster = 1;            // ... of the TMA-staged z pass
+  int ztx = 16;                // z pass tile: 16 x of one row (default), or 8 x of two rows y
   int zchunk = 0;              // > 0: the plane-local passes (y-inverse, x pass, y-forward) run chunk by chunk of this
                                // many z planes, so a chunk of the work buffer stays in L2 between them
   bool broken = false;
@@ -522,19 +526,21 @@ mvd_status y_pass_tma(mvd_ctx* c, float2* buf, int dir, int nz_planes, int xt0, 
 mvd_status z_conv_tma(mvd_ctx* c, const float2* in, float2* out, const float2* spec, int xt0, int n_xt) {
   const Plan& P = c->P;
   ZconvTmaArgs a{};
-  if (!make_map3(&a.in_map, in, P.Mx, P.My, P.N[2], P.Mx, P.plane, P.Tzt, 2, P.zbox) ||
-      !make_map3(&a.spec_map, spec, P.Mx, P.My, P.Mz, P.Mx, P.plane, P.Tzt, 2, P.zbox)) {
+  const int tx = c->ztx, ty = 2 * P.Tzt / tx;
+  n_xt = (P.Mx + tx - 1) / tx;
+  if (!make_map3(&a.in_map, in, P.Mx, P.My, P.N[2], P.Mx, P.plane, tx, ty, P.zbox) ||
+      !make_map3(&a.spec_map, spec, P.Mx, P.My, P.Mz, P.Mx, P.plane, tx, ty, P.zbox)) {
     snprintf(c->err, sizeof(c->err), "z pass: cuTensorMapEncodeTiled failed");
     c->broken = true;
     return MVD_ERR_CUDA;
   }
   a.out = out; a.tw = c->twz();
   a.T = P.Tzt; a.nthreads = P.ntzt; a.boxr = P.zbox; a.nbox = P.znbox;
-  a.xt0 = xt0; a.n_xt = n_xt;
+  a.xt0 = xt0; a.n_xt = n_xt; a.tx = tx;
   a.mx = P.Mx; a.my = P.My; a.plane = P.plane; a.nz = P.N[2]; a.nst_in = P.znst;
   if (c->zt_blocks == 0) c->zt_blocks = P.lz->zconv_tma_blocks_per_sm(a.nthreads, P.lz->zconv_tma_smem(a.T, a.boxr, a.nbox, a.nst_in));
   if (c->zt_blocks <= 0) { snprintf(c->err, sizeof(c->err), "z pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
-  a.grid = (int)std::min<long long>((long long)n_xt * ((P.My + 1) / 2), (long long)c->num_sms * c->zt_blocks);
+  a.grid = (int)std::min<long long>((long long)n_xt * ((P.My + ty - 1) / ty), (long long)c->num_sms * c->zt_blocks);
   a.cluster = c->zcluster;
   if (a.cluster > 1) {
     a.grid = a.grid / a.cluster * a.cluster;
@@ -614,6 +620,7 @@ XArgs x_args(mvd_ctx* c, const float2* in, float2* out, int rx) {
   a.psi = c->psi(); a.acc = c->acc(); a.partials = c->partials();
   a.eps = c->eps; a.psi_floor = c->psi_floor; a.inv_nviews = 1.0f / (float)P.V;
   a.tikhonov = c->tikhonov;
+  a.root_each = (!c->literal && P.V > kRootEachViews) ? 1 : 0;
   a.literal_product = c->literal;
   return a;
 }
@@ -1009,6 +1016,7 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
   c->y_tensor_store = env_int("MVD_YTSTORE", 0) ? 1 : 0;
   c->ycluster = std::min(8, std::max(1, env_int("MVD_YCLUSTER", 1)));
   c->zcluster = std::min(8, std::max(1, env_int("MVD_ZCLUSTER", 1)));
+  c->ztx = env_int("MVD_ZTX", 16) == 8 ? 8 : 16;   // 16 x 1 measured faster than 8 x 2 on configs 2-5
   c->zchunk = std::max(0, env_int("MVD_ZCHUNK", 0));
   if (c->zchunk > 0) c->zchunk = std::max(c->zchunk, (c->P.N[2] + kMaxZChunks - 1) / kMaxZChunks);
   if (c->use_graph && !c->stream) {   // the legacy default stream cannot be captured
@@ -1167,8 +1175,10 @@ mvd_status mvd_apply_product(mvd_ctx* c, int total_views) {
   if (c->broken) return MVD_ERR_STATE;
   const Plan& P = c->P;
   if (!P.combined) return MVD_ERR_UNSUPPORTED;
+  // with more than kRootEachViews views the factors were rooted one by one (x pass): no root left to take here
+  const int no_root = c->literal || (!c->literal && P.V > kRootEachViews);
   apply_product_kernel<<<P.sum_blocks, 256, 0, c->stream>>>(c->psi(), c->acc(), P.nvox, 1.0f / (float)total_views,
-                                                          c->literal, c->psi_floor, c->tikhonov, c->partials());
+                                                          no_root, c->psi_floor, c->tikhonov, c->partials());
   MVD_CK(cudaGetLastError(), "apply_product_kernel");
   ++c->launches;
   c->w_valid = false;

@@ -320,6 +320,10 @@ xrow_kernel(const XArgs p) {
             } else {
               float ft = p.literal_product ? vt : fmaxf(vt, 0.f);
               float fb = p.literal_product ? vb : fmaxf(vb, 0.f);
+              if (p.root_each) {
+                ft = __powf(ft, p.inv_nviews);
+                fb = __powf(fb, p.inv_nviews);
+              }
               if (p.acc_mode == ACC_MID || p.acc_mode == ACC_LAST) {
                 ft *= p.acc[it];
                 if (has_b) fb *= p.acc[ib];
@@ -328,9 +332,9 @@ xrow_kernel(const XArgs p) {
                 p.acc[it] = ft;
                 if (has_b) p.acc[ib] = fb;
               } else {
-                if (!p.literal_product && p.inv_nviews != 1.f) {
-                  ft = powf(ft, p.inv_nviews);
-                  fb = powf(fb, p.inv_nviews);
+                if (!p.literal_product && !p.root_each && p.inv_nviews != 1.f) {
+                  ft = __powf(ft, p.inv_nviews);
+                  fb = __powf(fb, p.inv_nviews);
                 }
                 const float o = p.psi[it];
                 const float nw = fmaxf(tikhonov_update(o * ft, p.tikhonov), p.psi_floor);

@@ -204,6 +204,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
           return nw;
         } else {                                                          // X_ACCUM (eq. 70 / 104, R1)
           float f = p.literal_product ? v : fmaxf(v, 0.f);
+          if (p.root_each) f = __powf(f, p.inv_nviews);                   // many views: root first, product after
           if (acc_read) f *= rrow[x];
           if constexpr (!acc_last) {
             arow[x] = f;
@@ -211,7 +212,7 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
           }
           // eq. 44: the |V|-th root as exp2(log2(f) / V) on the special-function unit (f is a product of V
           // ratios near 1: the hardware log2 / exp2 keep the relative error at a few 1e-7)
-          if (!p.literal_product && p.inv_nviews != 1.f) f = __powf(f, p.inv_nviews);
+          if (!p.literal_product && !p.root_each && p.inv_nviews != 1.f) f = __powf(f, p.inv_nviews);
           const float o = prow[x];
           float u = o * f;
           if constexpr (tik) u = tikhonov_value(u, p.tikhonov);           // R14
@@ -462,12 +463,15 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
 // and the spectrum tile [k][T] are both staged by tensor copies; the four register transforms
 // run in place on the input tile.
 // =========================================================================================
-template <int A, int B>
+template <int A, int B, int TX>
 __global__ void __launch_bounds__(PassCfg<A, B>::MAX_THREADS)
 zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
   constexpr int M = A * B;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  constexpr int TX = kTmaTile, T = 2 * kTmaTile;   // tile: 8 contiguous x of two consecutive rows y
+  // 16 columns per tile: TX = 8 contiguous x of two consecutive rows y, or TX = 16 x of one row (128-byte pieces:
+  // better for long pencils, where one CTA per SM is all that fits)
+  constexpr int T = 2 * kTmaTile, TY = T / TX;
+  static_assert(TX == 8 || TX == 16, "z tile: 8 x 2 or 16 x 1");
   const int NR = p.boxr * p.nbox;
   const int nst = p.nst_in;                                       // input stages: 1 or 2
   float2* buf = reinterpret_cast<float2*>(smem_raw);            // [nst][NR][T] input tiles
@@ -476,7 +480,7 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
   float2* tws = sbuf + (size_t)NR * T;                           // [B][AP]
   uint64_t* bars = reinterpret_cast<uint64_t*>(tws + B * AP);   // [0..1] input stages, [2] spectrum
   const int tid = threadIdx.x;
-  const int ny2 = (p.my + 1) / 2;                                 // row pairs
+  const int ny2 = (p.my + TY - 1) / TY;                           // row groups
   const int ntiles = p.n_xt * ny2;
 
   if (tid == 0) {
@@ -490,7 +494,7 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
 
   auto issue_in = [&](int tile, int s) {
     const int yp = tile / p.n_xt;
-    const int y = 2 * yp;
+    const int y = TY * yp;
     const int x0 = (p.xt0 + (tile - yp * p.n_xt)) * TX;
     mbar_expect_tx(&bars[s], (uint32_t)(NR * T * sizeof(float2)));
     for (int b = 0; b < p.nbox; ++b)
@@ -498,7 +502,7 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
   };
   auto issue_spec = [&](int tile) {
     const int yp = tile / p.n_xt;
-    const int y = 2 * yp;
+    const int y = TY * yp;
     const int x0 = (p.xt0 + (tile - yp * p.n_xt)) * TX;
     mbar_expect_tx(&bars[2], (uint32_t)(NR * T * sizeof(float2)));
     for (int b = 0; b < p.nbox; ++b)
@@ -524,10 +528,10 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
     // two input stages: the other stage was last read before the final barrier of the previous tile
     if (tid == 0 && more && nst == 2) issue_in(tile + (int)gridDim.x, s ^ 1);
     const int yp = tile / p.n_xt;
-    const int y = 2 * yp;
+    const int y = TY * yp;
     const int x0 = (p.xt0 + (tile - yp * p.n_xt)) * TX;
     const int xvalid = min(TX, p.mx - x0);
-    const int yvalid = min(2, p.my - y);
+    const int yvalid = min(TY, p.my - y);
     mbar_wait(&bars[s], nst == 2 ? ((it >> 1) & 1) : (it & 1));
 
     // F1: item (n2, x), forward A-point transforms over n1
@@ -628,7 +632,8 @@ struct LaunchTma {
     MVD_SET((strided_tma_kernel<A, B, 1, false>));
     MVD_SET((strided_tma_kernel<A, B, -1, true>));
     MVD_SET((strided_tma_kernel<A, B, 1, true>));
-    MVD_SET((zconv_tma_kernel<A, B>));
+    MVD_SET((zconv_tma_kernel<A, B, 8>));
+    MVD_SET((zconv_tma_kernel<A, B, 16>));
 #undef MVD_SET
     return cudaSuccess;
   }
@@ -675,7 +680,7 @@ struct LaunchTma {
   }
   static int zconv_blocks_per_sm(int nthreads, size_t smem) {
     int n = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, zconv_tma_kernel<A, B>, nthreads, smem);
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, zconv_tma_kernel<A, B, 8>, nthreads, smem);
     return e == cudaSuccess ? n : 0;
   }
   static cudaError_t strided(const StridedTmaArgs& a, int dir, cudaStream_t s) {
@@ -715,9 +720,11 @@ struct LaunchTma {
       at[0].val.clusterDim.z = 1;
       cfg.attrs = at;
       cfg.numAttrs = 1;
-      return cudaLaunchKernelEx(&cfg, zconv_tma_kernel<A, B>, a);
+      return a.tx == 16 ? cudaLaunchKernelEx(&cfg, zconv_tma_kernel<A, B, 16>, a)
+                        : cudaLaunchKernelEx(&cfg, zconv_tma_kernel<A, B, 8>, a);
     }
-    zconv_tma_kernel<A, B><<<a.grid, a.nthreads, smem, s>>>(a);
+    if (a.tx == 16) zconv_tma_kernel<A, B, 16><<<a.grid, a.nthreads, smem, s>>>(a);
+    else zconv_tma_kernel<A, B, 8><<<a.grid, a.nthreads, smem, s>>>(a);
     return cudaGetLastError();
   }
 

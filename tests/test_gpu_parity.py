@@ -212,6 +212,47 @@ def test_gpu_identical_views_equal_single_view(mvd, tiny):
     assert l2 < 3e-6 and mx < 1e-4
 
 
+def test_many_views_product_neither_overflows_nor_underflows(mvd, tiny):
+    """Combined variants keep a running fp32 product of the f_v.  With 40 views and an estimate far below (above) the
+    data every factor is ~30 (~1/30) and the bare product leaves the fp32 range; beyond 16 views the library roots
+    every factor before it enters the product.  Result: that of the oracle (P5: identical views == one view)."""
+    import torch
+    V = 40
+    p = _sub(tiny, [0] * V)
+    mean = float(np.mean(tiny.views[0], dtype=np.float64))
+    for scale in (1.0 / 30.0, 30.0):
+        psi0 = np.full(tiny.views[0].shape, mean * scale, np.float32)
+        for variant in ("independent", "efficient"):
+            d = mvd.Deconvolver(to_dev(p.views), p.psfs, variant=variant, psi0=torch.from_numpy(psi0).cuda())
+            d.iterate(1)
+            g1 = d.get_estimate_host()
+            d.iterate(2)
+            g3 = d.get_estimate_host()
+            d.close()
+            o = O.Oracle(p.views, p.psfs, variant, psi0=psi0)
+            o.iterate(1)
+            check(g1, o.psi, 1, "40 views %s x%g" % (variant, scale))
+            o.iterate(2)
+            check(g3, o.psi, 3, "40 views %s x%g" % (variant, scale))
+    # the view-parallel calls take the same guard (partial products of rooted factors, no root in apply_product)
+    views = to_dev(p.views)
+    psi0 = np.full(tiny.views[0].shape, mean / 30.0, np.float32)
+    ranks = [mvd.Deconvolver([views[v] for v in mvd.split_views(V, 2, r)], p.psfs, variant="independent",
+                             local_views=mvd.split_views(V, 2, r), psi0=torch.from_numpy(psi0).cuda()) for r in range(2)]
+    for d in ranks:
+        d.partial_product()
+    torch.cuda.synchronize()
+    prod = ranks[0].product_tensor() * ranks[1].product_tensor()
+    for d in ranks:
+        d.product_tensor().copy_(prod)
+        d.apply_product(V)
+    o = O.Oracle(p.views, p.psfs, "independent", psi0=psi0)
+    o.iterate(1)
+    check(ranks[0].get_estimate_host(), o.psi, 1, "40 views, view-parallel")
+    for d in ranks:
+        d.close()
+
+
 def test_gpu_delta_psf(mvd, tiny):
     """P6 (L851): delta PSFs: OSEM ends on the last view, combined on the geometric mean."""
     delta = np.zeros((3, 3, 3), np.float32)
