@@ -390,21 +390,24 @@ def run_ours(args):
             if args.blocked:
                 # the same sweep in block-wise mode, where the PSF half-size sets the halo and so the overhead (L240)
                 B, iters, reps = args.blocked, prob.iterations, []
-                for rep in range(2):                                   # first pass = warm-up
+                for rep in range(1 + max(1, args.repeats)):            # first pass = warm-up
                     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                     barrier()
                     e0.record(stream)
                     out, _ = mvd.deconvolve_blocked(dev_views, psfs, (B, B, B), iters, variant="osem", stream=stream)
                     e1.record(stream)
                     barrier()
-                    reps.append(e0.elapsed_time(e1))
+                    if rep:
+                        reps.append(e0.elapsed_time(e1))
                     del out
                 halo = [(b - 1) // 2 for b in box]
                 ext = float(np.prod([B + 2 * h for h in halo])) / B ** 3
-                sweep.append({"psf_box": list(box), "block": B, "halo": halo, "iterations": iters, "ms_total": reps[-1],
-                              "ms_per_step": reps[-1] / iters, "value": nvox * V * iters / (reps[-1] * 1e-3) / 1e9,
+                med = float(np.median(reps))
+                sweep.append({"psf_box": list(box), "block": B, "halo": halo, "iterations": iters, "ms_total": med,
+                              "ms_total_min_max": [min(reps), max(reps)],
+                              "ms_per_step": med / iters, "value": nvox * V * iters / (med * 1e-3) / 1e9,
                               "extended_over_central_voxels_interior_block": ext})
-                log("[bench] blocked sweep %s: %.1f ms" % (box, reps[-1]))
+                log("[bench] blocked sweep %s: %.1f ms" % (box, med))
                 continue
             d = mvd.Deconvolver(dev_views, psfs, variant="osem", stream=stream, use_graph=True)
             for _ in range(args.warmup):
@@ -663,7 +666,7 @@ def main():
                     help="what --gpus N ranks do (DESIGN.md section 10); default: N independent replicas of the OSEM workload")
     ap.add_argument("--blocked", type=int, default=0, metavar="B", help="config 5 as B^3 blocks + halo (mvd_deconvolve_blocked)")
     ap.add_argument("--psf-sweep", action="store_true", help="config 5 whole, one record per PSF box 9^3 ... 31x31x63")
-    ap.add_argument("--repeats", type=int, default=2, help="timed repeats of the blocked job (median)")
+    ap.add_argument("--repeats", type=int, default=3, help="timed repeats of the blocked job (median)")
     ap.add_argument("--sustained-s", type=float, default=3.0, help="seconds of back-to-back steps for the `sustained` leg (0 = skip)")
     ap.add_argument("--no-graph", action="store_true", help="time plain launches instead of one CUDA graph per iteration")
     ap.add_argument("--e2e-jobs", type=int, default=2)

@@ -120,7 +120,7 @@ struct XArgs {
   int complex_in;          // X_LOAD: rows of `in` are complex and transformed in full
   // TMA-staged variant (pass_tma.cuh)
   int real_stride;         // floats between real rows in shared memory
-  int bulk_real;           // real rows are 16-byte aligned: staged by bulk copies (else plain loads)
+  int bulk_real;           // real rows staged by bulk copies: 1 = rows 16-byte aligned, 2 = from the aligned address below each row; 0 = plain loads
   int grid;                // persistent CTAs
   int reverse;             // walk the tiles last to first
   int exch_stride;         // float2 per row of the exchange buffer (allocation)

@@ -16,6 +16,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <ctime>
 #include <new>
 #include <array>
 #include <vector>
@@ -305,7 +306,7 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
     if (P.lx->xrow_tma_smem(R, P.r[0], P.N[0], P.weighted) > 220 * 1024) P.xtma = 0;
     P.Rxt = R;
     P.ntxt = round_up32(R * ab);
-    int s = (P.N[0] + 3) / 4 * 4;
+    int s = (P.N[0] + 3 + 3) / 4 * 4;   // == xrow_rstride of pass_tma.cuh
     const int want = (P.lx->B % 32) / 4 * 4;
     while ((s % 32) != want) s += 4;
     P.xt_rstride = s;
@@ -372,6 +373,7 @@ struct mvd_ctx {
   int y_tensor_store = 0;      // y pass: results leave by tensor copies from the staged tile instead of per-thread stores
   int ycluster = 1;            // CTAs per cluster of the TMA-staged y pass (1 = plain launch)
   int zcluster = 1;            // ... of the TMA-staged z pass
+  int xbulk = 1;               // 0: real rows of the x pass by plain loads (MVD_XBULK=0, for comparison)
   int ztx = 16;                // z pass tile: 16 x of one row (default), or 8 x of two rows y
   int zchunk = 0;              // > 0: the plane-local passes (y-inverse, x pass, y-forward) run chunk by chunk of this
                                // many z planes, so a chunk of the work buffer stays in L2 between them
@@ -638,8 +640,10 @@ mvd_status x_pass(mvd_ctx* c, const XArgs& a_in, int mode) {
     a.reverse = c->use_flip ? (c->flip ^= 1) : 0;
     a.exch_stride = P.xt_exch; a.exch_stride_g = P.xt_exch_g; a.exch_stride_f = P.xt_exch_f;
     const float* real_src = mode == X_QUOT ? a.phi : (mode == X_ACCUM ? a.acc : a.psi);
-    a.bulk_real = (P.N[0] % 4 == 0) && ((reinterpret_cast<size_t>(real_src) & 15) == 0) &&
-                  ((reinterpret_cast<size_t>(a.wts) & 15) == 0);
+    // 1: every row of the real arrays is 16-byte aligned; 2: rows staged from the aligned address below them
+    a.bulk_real = ((P.N[0] % 4 == 0) && ((reinterpret_cast<size_t>(real_src) & 15) == 0) &&
+                   ((reinterpret_cast<size_t>(a.wts) & 15) == 0)) ? 1 : 2;
+    if (!c->xbulk) a.bulk_real = 0;
     const int flags = P.lx->xrow_tma_flags(a, mode) & 3;
     int& bl = c->xt_blocks[mode][flags];
     if (bl == 0) {
@@ -1016,6 +1020,7 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
   c->y_tensor_store = env_int("MVD_YTSTORE", 0) ? 1 : 0;
   c->ycluster = std::min(8, std::max(1, env_int("MVD_YCLUSTER", 1)));
   c->zcluster = std::min(8, std::max(1, env_int("MVD_ZCLUSTER", 1)));
+  c->xbulk = env_int("MVD_XBULK", 1);
   c->ztx = env_int("MVD_ZTX", 16) == 8 ? 8 : 16;   // 16 x 1 measured faster than 8 x 2 on configs 2-5
   c->zchunk = std::max(0, env_int("MVD_ZCHUNK", 0));
   if (c->zchunk > 0) c->zchunk = std::max(c->zchunk, (c->P.N[2] + kMaxZChunks - 1) / kMaxZChunks);
@@ -1520,6 +1525,15 @@ extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* vi
           ++launches;
         }
     if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { mvd_destroy(c); return MVD_ERR_CUDA; }
+    if (env_int("MVD_BLOCKED_TRACE", 0)) {
+      static double t_prev = 0.0;
+      timespec ts;
+      clock_gettime(CLOCK_MONOTONIC, &ts);
+      const double t = ts.tv_sec * 1e3 + ts.tv_nsec * 1e-6;
+      fprintf(stderr, "[mvd blocked] shape %dx%dx%d fft %dx%dx%d done, %.1f ms since the previous shape\n", d[0], d[1], d[2],
+              c->P.Mx, c->P.My, c->P.Mz, t_prev > 0.0 ? t - t_prev : 0.0);
+      t_prev = t;
+    }
     launches += mvd_launch_count(c);
     mvd_destroy(c);
   }

@@ -25,7 +25,8 @@ __host__ __device__ constexpr int xrow_cstride(int M, int A) {
   return s;
 }
 __host__ __device__ constexpr int xrow_rstride(int nx, int B) {
-  int s = (nx + 3) / 4 * 4;
+  int s = (nx + 3 + 3) / 4 * 4;   // + 3: a row whose global address is not 16-byte aligned is staged from the aligned
+                                  // address below it and sits up to 3 floats into its shared-memory row
   const int want = (B % 32) / 4 * 4;
   while ((s % 32) != want) s += 4;
   return s;
@@ -59,6 +60,11 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
   constexpr bool do_forward = MODE != X_ACCUM || acc_last;
   const bool need_real = MODE != X_ACCUM || acc_read;          // real rows staged at all
   const bool real_bulk = need_real && p.bulk_real, real_plain = need_real && !p.bulk_real;
+  // bulk_real == 2: rows of the real arrays start at addresses that are not multiples of 16 bytes (Nx not a multiple of
+  // 4, or a misaligned base).  A row is then staged from the aligned address below it (the copy also brings the last
+  // floats of the previous row and the first of the next) and read at an offset of `shift` floats; only the first
+  // and the last row of the array, whose aligned windows could leave it, are loaded with plain loads.
+  const bool shifted = real_bulk && p.bulk_real == 2;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int R = p.rows_per_cta;
   const int RSTR = p.real_stride;
@@ -80,6 +86,10 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
   const float* real_src = MODE == X_QUOT ? p.phi : (MODE == X_ACCUM ? p.acc : p.psi);
   const int ntiles = (int)((p.nrows + R - 1) / R);
   const int nrows_i = (int)p.nrows;
+  const unsigned mis_r = shifted ? (unsigned)((reinterpret_cast<uintptr_t>(real_src) >> 2) & 3u) : 0u;
+  const unsigned mis_w = (shifted && has_w) ? (unsigned)((reinterpret_cast<uintptr_t>(p.wts) >> 2) & 3u) : 0u;
+  auto row_shift = [&](unsigned mis, int g) { return (int)((mis + (unsigned)g * (unsigned)p.nx) & 3u); };
+  auto row_staged = [&](int a, int g) { return (g > 0 || a == 0) && (g < nrows_i - 1 || ((a + p.nx) & 3) == 0); };
 
   if (tid == 0) {
     mbar_init(&bars[0], 1);   // complex rows landed
@@ -106,11 +116,37 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
     const int tile = p.reverse ? ntiles - 1 - t : t;
     const int row0 = tile * R;
     const int rv = min(R, nrows_i - row0);
-    if (tid == 0) mbar_expect_tx(&bars[1], (uint32_t)rv * (uint32_t)(p.nx * sizeof(float)) * (has_w ? 2u : 1u));
+    if (!shifted) {
+      if (tid == 0) mbar_expect_tx(&bars[1], (uint32_t)rv * (uint32_t)(p.nx * sizeof(float)) * (has_w ? 2u : 1u));
+      __syncwarp();
+      for (int r = tid; r < rv; r += 32) {
+        bulk_g2s(rst + (size_t)r * RSTR, real_src + (long long)(row0 + r) * p.nx, p.nx * sizeof(float), &bars[1]);
+        if (has_w) bulk_g2s(wrst + (size_t)r * RSTR, p.wts + (long long)(row0 + r) * p.nx, p.nx * sizeof(float), &bars[1]);
+      }
+      return;
+    }
+    uint32_t bytes = 0;
+    for (int r = tid; r < rv; r += 32) {
+      const int g = row0 + r, a = row_shift(mis_r, g);
+      if (row_staged(a, g)) bytes += (uint32_t)(((a + p.nx) * 4 + 15) & ~15);
+      if (has_w) {
+        const int aw = row_shift(mis_w, g);
+        if (row_staged(aw, g)) bytes += (uint32_t)(((aw + p.nx) * 4 + 15) & ~15);
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
+    if (tid == 0) mbar_expect_tx(&bars[1], bytes);
     __syncwarp();
     for (int r = tid; r < rv; r += 32) {
-      bulk_g2s(rst + (size_t)r * RSTR, real_src + (long long)(row0 + r) * p.nx, p.nx * sizeof(float), &bars[1]);
-      if (has_w) bulk_g2s(wrst + (size_t)r * RSTR, p.wts + (long long)(row0 + r) * p.nx, p.nx * sizeof(float), &bars[1]);
+      const int g = row0 + r, a = row_shift(mis_r, g);
+      if (row_staged(a, g))
+        bulk_g2s(rst + (size_t)r * RSTR, real_src + (long long)g * p.nx - a, (uint32_t)(((a + p.nx) * 4 + 15) & ~15), &bars[1]);
+      if (has_w) {
+        const int aw = row_shift(mis_w, g);
+        if (row_staged(aw, g))
+          bulk_g2s(wrst + (size_t)r * RSTR, p.wts + (long long)g * p.nx - aw, (uint32_t)(((aw + p.nx) * 4 + 15) & ~15), &bars[1]);
+      }
     }
   };
 
@@ -130,7 +166,20 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
     const bool actA = tid < R * A && growA < nrows_i;
     const bool actB = tid < R * B && growB < nrows_i;
     const bool more = tile + (int)gridDim.x < ntiles;
-    if (real_plain) {   // rows not 16-byte aligned: plain loads of this tile's real rows
+    if (shifted) {      // the first / last row of the array: plain loads into the same shifted position
+      const int rv = min(R, nrows_i - row0);
+      for (int r = 0; r < rv; ++r) {
+        const int g = row0 + r, a = row_shift(mis_r, g);
+        if (!row_staged(a, g))
+          for (int x = tid; x < p.nx; x += blockDim.x) rst[(size_t)r * RSTR + a + x] = real_src[(long long)g * p.nx + x];
+        if (has_w) {
+          const int aw = row_shift(mis_w, g);
+          if (!row_staged(aw, g))
+            for (int x = tid; x < p.nx; x += blockDim.x) wrst[(size_t)r * RSTR + aw + x] = p.wts[(long long)g * p.nx + x];
+        }
+      }
+    }
+    if (real_plain) {   // staging by bulk copies switched off (MVD_XBULK=0): plain loads of this tile's real rows
       const int rv = min(R, nrows_i - row0);
       for (int i = tid; i < rv * p.nx; i += blockDim.x) {
         const int r = i / p.nx, x = i - r * p.nx;
@@ -182,8 +231,8 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
     // ---- pointwise stage on the real row -------------------------------------------------------
     if (actB) {
       const long long rbase = (long long)growB * p.nx;
-      const float* rrow = rst + (size_t)rowB * RSTR;
-      const float* wrow = wrst + (size_t)rowB * RSTR;
+      const float* rrow = rst + (size_t)rowB * RSTR + (shifted ? row_shift(mis_r, growB) : 0);
+      const float* wrow = wrst + (size_t)rowB * RSTR + (shifted ? row_shift(mis_w, growB) : 0);
       float* prow = p.psi + rbase;
       float* arow = p.acc + rbase;
       const int lo_int = p.rx, hi_int = min(p.hx - p.rx, p.nx - p.hx);   // interior: no overlap, both halves live
