@@ -17,6 +17,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <ctime>
+#include <mutex>
 #include <new>
 #include <array>
 #include <vector>
@@ -768,6 +769,30 @@ mvd_status ensure_w(mvd_ctx* c) {
   return MVD_OK;
 }
 
+// ---- pinned staging buffer of the PSF taps (process-wide, grow-only) -----------------------------
+std::mutex g_staging_mutex;
+char* g_staging = nullptr;
+size_t g_staging_bytes = 0;
+
+char* staging_acquire(size_t bytes) {
+  g_staging_mutex.lock();
+  if (bytes > g_staging_bytes) {
+    if (g_staging) cudaFreeHost(g_staging);
+    g_staging = nullptr;
+    g_staging_bytes = 0;
+    const size_t want = std::max(bytes, (size_t)1 << 20);
+    if (cudaHostAlloc(reinterpret_cast<void**>(&g_staging), want, cudaHostAllocMapped | cudaHostAllocPortable) != cudaSuccess) {
+      cudaGetLastError();
+      g_staging = nullptr;
+      g_staging_mutex.unlock();
+      return nullptr;
+    }
+    g_staging_bytes = want;
+  }
+  return g_staging;
+}
+void staging_release() { g_staging_mutex.unlock(); }
+
 // ---- precompute (S0) ---------------------------------------------------------------------------
 mvd_status build_spectrum(mvd_ctx* c, const double* kern, Dims3 K, float2* spec) {
   const Plan& P = c->P;
@@ -821,7 +846,11 @@ mvd_status precompute(mvd_ctx* c, const float* const* psfs_host, const double* s
   {
     size_t total = 0;
     for (int v = 0; v < P.V; ++v) total += align_up((size_t)P.K[v].x * P.K[v].y * P.K[v].z * sizeof(float), 256);
-    MVD_CK(cudaHostAlloc(reinterpret_cast<void**>(&c->psf_staging), total, cudaHostAllocMapped), "pinned PSF staging");
+    // one grow-only pinned buffer per process, handed from one mvd_create to the next (allocating and freeing
+    // mapped pinned memory per context cost tens of milliseconds now and then: the block-wise mode creates a context
+    // per block shape); held under a lock until this mvd_create has synchronised its stream
+    c->psf_staging = staging_acquire(total);
+    if (!c->psf_staging) { snprintf(c->err, sizeof(c->err), "pinned PSF staging: allocation failed"); return MVD_ERR_CUDA; }
     char* dev_base = nullptr;
     MVD_CK(cudaHostGetDevicePointer(reinterpret_cast<void**>(&dev_base), c->psf_staging, 0), "pinned PSF staging");
     size_t off = 0;
@@ -1063,7 +1092,7 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
   if (s == MVD_OK && c->fail(cudaStreamSynchronize(c->stream), "mvd_create")) s = MVD_ERR_CUDA;
   if (c->psf_staging) {
     if (s != MVD_OK) cudaStreamSynchronize(c->stream);   // a kernel may still be reading the staged taps
-    cudaFreeHost(c->psf_staging);
+    staging_release();
     c->psf_staging = nullptr;
   }
   if (s != MVD_OK) {
