@@ -162,6 +162,64 @@ __global__ void __launch_bounds__(256) corr_crop_mul_kernel(const double* __rest
   }
 }
 
+// The same product, register-tiled: one block per output row (jz, jy); a thread owns TJ = 4 consecutive taps jx and a
+// share of the (uz, uy) rows of the sum, and slides a window of 4 values of G along ux, so every step costs one load
+// of G, one of P_v and four fp64 FMAs (the kernel above: two loads per FMA).  Partial sums of the row shares are
+// added through shared memory.  Needs ceil(Kx / 4) <= blockDim.x.
+// General form: out[j] (op)= sum_u Pv[K-1-u] G[o + j - u] for j in the box J, G zero outside Gd; op is '*=' (the
+// cropped factors of eq. 105 / 107: J = K, o = (Gd-1)/2) or '=' (assign: with G = P_w, J = 2K-1, o = 0 this is the
+// autocorrelation P_w (*) P_w*, which is symmetric, so the mirrored index order does not matter).
+__global__ void __launch_bounds__(128) corr_crop_mul_tiled_kernel(const double* __restrict__ Pv, Dims3 K,
+                                                                  const double* __restrict__ G, Dims3 Gd,
+                                                                  double* __restrict__ kern, Dims3 J, Dims3 o,
+                                                                  int assign) {
+  constexpr int TJ = 4;
+  __shared__ double red[128 * TJ];
+  const int nxt = (J.x + TJ - 1) / TJ;
+  const int parts = blockDim.x / nxt;
+  const int part = threadIdx.x / nxt, xt = threadIdx.x - part * nxt;
+  const int jy = blockIdx.x % J.y, jz = blockIdx.x / J.y;
+  const int oy = o.y + jy, oz = o.z + jz;
+  const int base = o.x + xt * TJ;                        // index into a G row of tap jx0 = xt * TJ at ux = 0
+  double acc[TJ] = {0.0, 0.0, 0.0, 0.0};
+  if (part < parts) {
+    const int nrows = K.z * K.y;
+    for (int r = part; r < nrows; r += parts) {
+      const int uz = r / K.y, uy = r - uz * K.y;
+      const int gz = oz - uz, gy = oy - uy;
+      if (gz < 0 || gz >= Gd.z || gy < 0 || gy >= Gd.y) continue;
+      const double* pv = Pv + ((long long)(K.z - 1 - uz) * K.y + (K.y - 1 - uy)) * K.x + (K.x - 1);   // pv[-ux] = flipped tap ux
+      const double* g = G + ((long long)gz * Gd.y + gy) * Gd.x;
+      double w[TJ];
+#pragma unroll
+      for (int t = 0; t < TJ; ++t) {
+        const int i = base + t;
+        w[t] = (i >= 0 && i < Gd.x) ? g[i] : 0.0;
+      }
+#pragma unroll 4
+      for (int ux = 0; ux < K.x; ++ux) {
+        const double pval = pv[-ux];
+#pragma unroll
+        for (int t = 0; t < TJ; ++t) acc[t] = fma(pval, w[t], acc[t]);
+#pragma unroll
+        for (int t = TJ - 1; t > 0; --t) w[t] = w[t - 1];
+        const int i = base - ux - 1;
+        w[0] = (i >= 0 && i < Gd.x) ? g[i] : 0.0;
+      }
+    }
+  }
+#pragma unroll
+  for (int t = 0; t < TJ; ++t) red[threadIdx.x * TJ + t] = acc[t];
+  __syncthreads();
+  if ((int)threadIdx.x < J.x) {
+    const int jx = threadIdx.x;
+    double sum = 0.0;
+    for (int q = 0; q < parts; ++q) sum += red[(q * nxt + jx / TJ) * TJ + (jx % TJ)];
+    double* dst = kern + ((long long)jz * J.y + jy) * J.x + jx;
+    *dst = assign ? sum : *dst * sum;
+  }
+}
+
 // kern[j] = (P[K-1-j])^power  (mirror, L312; power = V gives eq. 108, R9)
 __global__ void flip_pow_kernel(const double* __restrict__ P, Dims3 K, int power,
                                 double* __restrict__ kern) {

@@ -374,6 +374,7 @@ struct mvd_ctx {
   int y_tensor_store = 0;      // y pass: results leave by tensor copies from the staged tile instead of per-thread stores
   int ycluster = 1;            // CTAs per cluster of the TMA-staged y pass (1 = plain launch)
   int zcluster = 1;            // ... of the TMA-staged z pass
+  int corr_tiled = 1;          // 0: the untiled fp64 correlation kernel of the precompute (MVD_CORR_TILED=0)
   int xbulk = 1;               // 0: real rows of the x pass by plain loads (MVD_XBULK=0, for comparison)
   int ztx = 16;                // z pass tile: 16 x of one row (default), or 8 x of two rows y
   int zchunk = 0;              // > 0: the plane-local passes (y-inverse, x pass, y-forward) run chunk by chunk of this
@@ -803,19 +804,31 @@ mvd_status build_spectrum(mvd_ctx* c, const double* kern, Dims3 K, float2* spec)
                                                                         Dims3{P.Mx, P.My, P.Mz}, scale);
   MVD_CK(cudaGetLastError(), "scatter_kernel");
   ++c->launches;
-  // x: complex rows, all My*Mz of them, in place
-  XArgs a = x_args(c, spec, spec, 0);
-  a.nrows = (long long)P.My * P.Mz;
-  a.ny_rows = P.My;
-  a.complex_in = 1;
-  MVD_TRY(x_pass(c, a, X_LOAD));
-  // y: every plane of the Mz, full pencils
-  {
+  // The taps sit (wrapped) in the planes z in [0, cz] and [Mz-cz, Mz) and, there, in the rows y in [0, cy] and
+  // [My-cy, My): the x pass only visits those rows, the y pass only those planes; the z pass sees the whole buffer.
+  const int cz = (K.z - 1) / 2, cy = (K.y - 1) / 2;
+  int zr[2][2] = {{0, std::min(cz + 1, P.Mz)}, {std::max(P.Mz - cz, cz + 1), P.Mz}};   // [z0, z1)
+  int yr[2][2] = {{0, std::min(cy + 1, P.My)}, {std::max(P.My - cy, cy + 1), P.My}};
+  for (int iz = 0; iz < 2; ++iz) {
+    const int z0 = zr[iz][0], nz = zr[iz][1] - z0;
+    if (nz <= 0) continue;
+    float2* zbase = spec + (long long)z0 * P.plane;
+    // x: complex rows, in place
+    for (int iy = 0; iy < 2; ++iy) {
+      const int y0 = yr[iy][0], ny = yr[iy][1] - y0;
+      if (ny <= 0) continue;
+      XArgs a = x_args(c, zbase + (long long)y0 * P.Mx, zbase + (long long)y0 * P.Mx, 0);
+      a.nrows = (long long)ny * nz;
+      a.ny_rows = ny;
+      a.complex_in = 1;
+      MVD_TRY(x_pass(c, a, X_LOAD));
+    }
+    // y: full pencils of these planes
     StridedArgs s{};
-    s.in = spec; s.out = spec; s.tw = c->twy();
+    s.in = zbase; s.out = zbase; s.tw = c->twy();
     s.T = P.Tys; s.nthreads = P.ntys;
     s.line_len = P.Mx; s.tiles_per_line = (P.Mx + s.T - 1) / s.T;
-    s.n_outer = P.Mz;
+    s.n_outer = nz;
     s.in_outer_stride = s.out_outer_stride = P.plane;
     s.in_pstride = s.out_pstride = P.Mx;
     s.n_in = P.My; s.n_out = P.My;
@@ -880,7 +893,11 @@ mvd_status precompute(mvd_ctx* c, const float* const* psfs_host, const double* s
     for (int w = 0; w < P.V; ++w) {
       const Dims3 K = P.K[w];
       const long long tot = (long long)(2 * K.x - 1) * (2 * K.y - 1) * (2 * K.z - 1);
-      autocorr_kernel<<<(unsigned)((tot + 127) / 128), 128, 0, c->stream>>>(c->psf(w), K, c->autoc(w));
+      if (2 * K.x - 1 <= 128 && c->corr_tiled)   // P_w (*) P_w* = sum_u P[K-1-u] P[m - u] read backwards (symmetric)
+        corr_crop_mul_tiled_kernel<<<(unsigned)((2 * K.y - 1) * (2 * K.z - 1)), 128, 0, c->stream>>>(
+            c->psf(w), K, c->psf(w), K, c->autoc(w), Dims3{2 * K.x - 1, 2 * K.y - 1, 2 * K.z - 1}, Dims3{0, 0, 0}, 1);
+      else
+        autocorr_kernel<<<(unsigned)((tot + 127) / 128), 128, 0, c->stream>>>(c->psf(w), K, c->autoc(w));
       MVD_CK(cudaGetLastError(), "autocorr_kernel");
       ++c->launches;
     }
@@ -897,11 +914,13 @@ mvd_status precompute(mvd_ctx* c, const float* const* psfs_host, const double* s
       for (int w = 0; w < P.V; ++w) {
         if (w == v) continue;
         const Dims3 Kw = P.K[w];
-        if (P.kmode == MVD_KERNEL_COMPOUND)
-          corr_crop_mul_kernel<<<g128, 256, 0, c->stream>>>(c->psf(v), K, c->autoc(w),
-                                                            Dims3{2 * Kw.x - 1, 2 * Kw.y - 1, 2 * Kw.z - 1}, c->kern(v));
+        const double* gsrc = P.kmode == MVD_KERNEL_COMPOUND ? c->autoc(w) : c->psf(w);
+        const Dims3 gd = P.kmode == MVD_KERNEL_COMPOUND ? Dims3{2 * Kw.x - 1, 2 * Kw.y - 1, 2 * Kw.z - 1} : Kw;
+        if (K.x <= 128 && c->corr_tiled)
+          corr_crop_mul_tiled_kernel<<<(unsigned)(K.y * K.z), 128, 0, c->stream>>>(
+              c->psf(v), K, gsrc, gd, c->kern(v), K, Dims3{(gd.x - 1) / 2, (gd.y - 1) / 2, (gd.z - 1) / 2}, 0);
         else
-          corr_crop_mul_kernel<<<g128, 256, 0, c->stream>>>(c->psf(v), K, c->psf(w), Kw, c->kern(v));
+          corr_crop_mul_kernel<<<g128, 256, 0, c->stream>>>(c->psf(v), K, gsrc, gd, c->kern(v));
         MVD_CK(cudaGetLastError(), "corr_crop_mul_kernel");
         ++c->launches;
       }
@@ -1049,6 +1068,7 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
   c->y_tensor_store = env_int("MVD_YTSTORE", 0) ? 1 : 0;
   c->ycluster = std::min(8, std::max(1, env_int("MVD_YCLUSTER", 1)));
   c->zcluster = std::min(8, std::max(1, env_int("MVD_ZCLUSTER", 1)));
+  c->corr_tiled = env_int("MVD_CORR_TILED", 1);
   c->xbulk = env_int("MVD_XBULK", 1);
   c->ztx = env_int("MVD_ZTX", 16) == 8 ? 8 : 16;   // 16 x 1 measured faster than 8 x 2 on configs 2-5
   c->zchunk = std::max(0, env_int("MVD_ZCHUNK", 0));
