@@ -566,9 +566,11 @@ def run_ours(args):
         barrier()                                      # the first-use iterations have read the view buffers
 
         def stream_series(n):
-            pending = None
+            pending, done = None, None
             for i in range(n):
                 dd, bufs = ctxs[i % 2]
+                if done is not None:                   # one time-point's kernels at a time: the other context's stream
+                    dd.stream.wait_event(done)         # starts when the previous time-point's iterations have finished
                 with torch.cuda.stream(copy_stream):
                     for b, h in zip(bufs, host_views):
                         b.copy_(h, non_blocking=True)
@@ -576,6 +578,8 @@ def run_ours(args):
                     ready.record(copy_stream)
                 dd.restart(ready)
                 dd.iterate(iters)
+                done = torch.cuda.Event()
+                done.record(dd.stream)
                 if pending is not None:                # blocks until time-point i-1 is done and copied out
                     pending[0].get_estimate_host(pending[1].numpy())
                 pending = (dd, outs[i % 2])

@@ -16,7 +16,6 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
-#include <ctime>
 #include <mutex>
 #include <new>
 #include <array>
@@ -1574,15 +1573,6 @@ extern "C" mvd_status mvd_deconvolve_blocked(int n_views, const float* const* vi
           ++launches;
         }
     if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { mvd_destroy(c); return MVD_ERR_CUDA; }
-    if (env_int("MVD_BLOCKED_TRACE", 0)) {
-      static double t_prev = 0.0;
-      timespec ts;
-      clock_gettime(CLOCK_MONOTONIC, &ts);
-      const double t = ts.tv_sec * 1e3 + ts.tv_nsec * 1e-6;
-      fprintf(stderr, "[mvd blocked] shape %dx%dx%d fft %dx%dx%d done, %.1f ms since the previous shape\n", d[0], d[1], d[2],
-              c->P.Mx, c->P.My, c->P.Mz, t_prev > 0.0 ? t - t_prev : 0.0);
-      t_prev = t;
-    }
     launches += mvd_launch_count(c);
     mvd_destroy(c);
   }
