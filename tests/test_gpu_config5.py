@@ -9,7 +9,8 @@ exact and small (VERDICT r1 "Next round" 1c/1d):
   problems, so this is the full definition of the blocked result there).
 * whole volume: one full iteration (6 sequential view-updates, eq. 109-112) is compared on sub-volumes
   with the oracle run on a crop that holds the sub-volume plus the dependence radius of the iteration
-  (2r per view-update, 12r for six: 144 voxels in x and y, 300 in z, so the crop spans all of z).
+  (2r per view-update, 12r for six: 144 voxels in x and y, 300 in z, so the crop spans all of z; the combined
+  variants take every f_v from the same estimate, so one of their iterations reaches 2r only and two reach 4r).
   Inside that margin the crop's artificial zero extension cannot reach the sub-volume, so the
   oracle's values there are those of the whole-volume iteration.  One sub-volume sits at a volume
   corner, the other straddles the half-row seam x = Nx/2 of the packed x transform and a y face.
@@ -105,3 +106,33 @@ def test_config5_whole_volume_iteration_on_sub_volumes(mvd, config5):
         o.iterate(1)
         ref = o.psi[:, y0 - cy0:y0 - cy0 + S, x0 - cx0:x0 - cx0 + S]
         check(g[:, y0:y0 + S, x0:x0 + S], ref, 1, "config 5 whole, sub-volume at y=%d x=%d" % (y0, x0))
+
+
+@pytest.mark.parametrize("variant", ["efficient", "independent"])
+def test_config5_whole_volume_combined_variants_on_sub_volumes(mvd, config5, variant):
+    """eq. 70 / 104 at 1024x1024x512: two iterations of the combined variants (shared forward pass, product
+    accumulation over 6 views, root) against the oracle on crops with a margin of 4r (the reach of two iterations)."""
+    import torch
+    p = config5
+    nz, ny, nx = p.views[0].shape
+    views = to_dev(p.views)
+    d = mvd.Deconvolver(views, p.psfs, variant=variant)
+    d.iterate(2)
+    g = d.get_estimate_host()
+    d.close()
+    del views, d
+    torch.cuda.empty_cache()
+    assert np.isfinite(g).all()
+    rz, ry, rx = [(k - 1) // 2 for k in p.psfs[0].shape]
+    mz, my, mx = 4 * rz, 4 * ry, 4 * rx
+    psi0 = _whole_mean(p.views)
+    S = 64
+    for (z0, y0, x0) in ((0, 0, 0), (nz // 2 - S // 2, ny - S, nx // 2 - S // 2)):
+        cz0, cz1 = max(z0 - mz, 0), min(z0 + S + mz, nz)
+        cy0, cy1 = max(y0 - my, 0), min(y0 + S + my, ny)
+        cx0, cx1 = max(x0 - mx, 0), min(x0 + S + mx, nx)
+        sub = [v[cz0:cz1, cy0:cy1, cx0:cx1] for v in p.views]
+        o = O.Oracle(sub, p.psfs, variant, psi0=np.full(sub[0].shape, psi0))
+        o.iterate(2)
+        ref = o.psi[z0 - cz0:z0 - cz0 + S, y0 - cy0:y0 - cy0 + S, x0 - cx0:x0 - cx0 + S]
+        check(g[z0:z0 + S, y0:y0 + S, x0:x0 + S], ref, 2, "config 5 %s, sub-volume at %s" % (variant, (z0, y0, x0)))
