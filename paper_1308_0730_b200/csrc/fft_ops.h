@@ -22,6 +22,7 @@ __host__ __device__ constexpr int strided_tma_tile(int M) { return (M > 500 && M
 struct StridedTmaArgs {
   CUtensorMap in_map;      // dims (x: line_len, pencil: n_in, outer: n_outer); box (T, boxr, 1)
   CUtensorMap out_map;     // tensor_store: dims (x: line_len, pencil: n_out, outer: n_outer); same box
+  int pair;                // 1: two adjacent columns per thread, 128-bit accesses (needs even line_len and T)
   int tensor_store;        // 1: results go back into the staged tile and leave by tensor copies (rows >= n_out clipped)
   float2* out;
   const float2* tw;        // tw[j] = exp(-2*pi*i*j/M)

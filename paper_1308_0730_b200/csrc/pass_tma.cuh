@@ -368,9 +368,21 @@ constexpr int strided_tma_threads() {
   return t < PassCfg<A, B>::MAX_THREADS ? t : PassCfg<A, B>::MAX_THREADS;
 }
 
-template <int A, int B, int DIR, bool TS>
-__global__ void __launch_bounds__(TS ? strided_tma_threads<A, B>() : PassCfg<A, B>::MAX_THREADS, TS ? 2 : 0)
+// VAR: 0 = per-thread stores, 1 = TS (tensor stores, above), 2 = PAIR: a thread transforms two adjacent columns at once,
+// so every shared-memory and global access is 128 bits wide (half the load / store / address instructions, half the
+// threads, twice the independent work per thread).
+template <int A, int B>
+constexpr int strided_tma_pair_threads() {
+  constexpr int items = strided_tma_tile(A * B) / 2 * PassCfg<A, B>::AB_MAX;
+  constexpr int t = (items + 31) / 32 * 32;
+  return t < 512 ? t : 512;
+}
+template <int A, int B, int DIR, int VAR>
+__global__ void __launch_bounds__(VAR == 1 ? strided_tma_threads<A, B>() : (VAR == 2 ? strided_tma_pair_threads<A, B>() : PassCfg<A, B>::MAX_THREADS),
+                                  VAR == 1 ? 2 : 0)
 strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
+  constexpr bool TS = VAR == 1;
+  constexpr bool PAIR = VAR == 2;
   constexpr int M = A * B;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int T = strided_tma_tile(M);
@@ -423,22 +435,48 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
     const int xvalid = min(T, p.line_len - x0);
     mbar_wait(&bars[s], nst == 2 ? ((it >> 1) & 1) : (it & 1));
 
+    if constexpr (PAIR) {
+      constexpr int H = T / 2;                     // float4 (two complex) per tile row
+      float4* sm4 = reinterpret_cast<float4*>(sm);
+      for (int i = tid; i < H * B; i += blockDim.x) {
+        const int n2 = i / H;
+        float2 v0[A], v1[A];
+        static_for<0, A>([&](auto n1_) {
+          constexpr int n1 = decltype(n1_)::value;
+          const float4 q = sm4[n1 * B * H + i];
+          v0[n1] = make_float2(q.x, q.y);
+          v1[n1] = make_float2(q.z, q.w);
+        });
+        FftReg<A, DIR>::run(v0);
+        FftReg<A, DIR>::run(v1);
+        static_for<0, A>([&](auto k1_) {
+          constexpr int k1 = decltype(k1_)::value;
+          if constexpr (k1 > 0) {
+            const float2 w = tws[n2 * AP + k1];
+            v0[k1] = DIR < 0 ? cmul(v0[k1], w) : cmul_conj(v0[k1], w);
+            v1[k1] = DIR < 0 ? cmul(v1[k1], w) : cmul_conj(v1[k1], w);
+          }
+          sm4[k1 * B * H + i] = make_float4(v0[k1].x, v0[k1].y, v1[k1].x, v1[k1].y);
+        });
+      }
+    } else {
     for (int i = tid; i < T * B; i += blockDim.x) {
-      const int n2 = i / T;
-      float2 v[A];
-      static_for<0, A>([&](auto n1_) {
-        constexpr int n1 = decltype(n1_)::value;
-        v[n1] = sm[n1 * B * T + i];
-      });
-      FftReg<A, DIR>::run(v);
-      static_for<0, A>([&](auto k1_) {
-        constexpr int k1 = decltype(k1_)::value;
-        if constexpr (k1 > 0) {
-          const float2 w = tws[n2 * AP + k1];
-          v[k1] = DIR < 0 ? cmul(v[k1], w) : cmul_conj(v[k1], w);
-        }
-        sm[k1 * B * T + i] = v[k1];
-      });
+        const int n2 = i / T;
+        float2 v[A];
+        static_for<0, A>([&](auto n1_) {
+          constexpr int n1 = decltype(n1_)::value;
+          v[n1] = sm[n1 * B * T + i];
+        });
+        FftReg<A, DIR>::run(v);
+        static_for<0, A>([&](auto k1_) {
+          constexpr int k1 = decltype(k1_)::value;
+          if constexpr (k1 > 0) {
+            const float2 w = tws[n2 * AP + k1];
+            v[k1] = DIR < 0 ? cmul(v[k1], w) : cmul_conj(v[k1], w);
+          }
+          sm[k1 * B * T + i] = v[k1];
+        });
+      }
     }
     __syncthreads();
     if constexpr (TS) {
@@ -476,6 +514,35 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
           issue(tile + (int)gridDim.x, 0);
         }
       }
+    } else if constexpr (PAIR) {
+      constexpr int H = T / 2;
+      const float4* sm4 = reinterpret_cast<const float4*>(sm);
+      float2* out = p.out + (long long)outer * p.out_outer_stride + x0;
+      for (int j = tid; j < H * A; j += blockDim.x) {
+        const int k1 = j / H;
+        const int xp = j - k1 * H;
+        float2 u0[B], u1[B];
+        static_for<0, B>([&](auto n2_) {
+          constexpr int n2 = decltype(n2_)::value;
+          const float4 q = sm4[(k1 * B + n2) * H + xp];
+          u0[n2] = make_float2(q.x, q.y);
+          u1[n2] = make_float2(q.z, q.w);
+        });
+        FftReg<B, DIR>::run(u0);
+        FftReg<B, DIR>::run(u1);
+        if (2 * xp < xvalid) {                     // line_len and T are even: a pair is valid or not as a whole
+          float4* o = reinterpret_cast<float4*>(out + (long long)k1 * p.out_pstride + 2 * xp);
+          static_for<0, B>([&](auto k2_) {
+            constexpr int k2 = decltype(k2_)::value;
+            if (k1 + A * k2 < p.n_out)
+              *reinterpret_cast<float4*>(reinterpret_cast<float2*>(o) + (long long)(A * k2) * p.out_pstride) =
+                  make_float4(u0[k2].x, u0[k2].y, u1[k2].x, u1[k2].y);
+          });
+        }
+      }
+      fence_proxy_async();
+      __syncthreads();
+      if (tid == 0 && more && nst == 1) issue(tile + (int)gridDim.x, 0);
     } else {
       float2* out = p.out + (long long)outer * p.out_outer_stride + x0;
       for (int j = tid; j < T * A; j += blockDim.x) {
@@ -677,10 +744,12 @@ struct LaunchTma {
     MVD_SET((xrow_tma_kernel<A, B, X_ACCUM, 0>));
     MVD_SET((xrow_tma_kernel<A, B, X_ACCUM, XF_LAST>));
     MVD_SET((xrow_tma_kernel<A, B, X_ACCUM, XF_LAST | XF_TIK>));
-    MVD_SET((strided_tma_kernel<A, B, -1, false>));
-    MVD_SET((strided_tma_kernel<A, B, 1, false>));
-    MVD_SET((strided_tma_kernel<A, B, -1, true>));
-    MVD_SET((strided_tma_kernel<A, B, 1, true>));
+    MVD_SET((strided_tma_kernel<A, B, -1, 0>));
+    MVD_SET((strided_tma_kernel<A, B, 1, 0>));
+    MVD_SET((strided_tma_kernel<A, B, -1, 1>));
+    MVD_SET((strided_tma_kernel<A, B, 1, 1>));
+    MVD_SET((strided_tma_kernel<A, B, -1, 2>));
+    MVD_SET((strided_tma_kernel<A, B, 1, 2>));
     MVD_SET((zconv_tma_kernel<A, B, 8>));
     MVD_SET((zconv_tma_kernel<A, B, 16>));
 #undef MVD_SET
@@ -723,8 +792,8 @@ struct LaunchTma {
   static int strided_blocks_per_sm(int dir, int nthreads, size_t smem) {
     int n = 0;
     cudaError_t e = dir < 0
-        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, strided_tma_kernel<A, B, -1, false>, nthreads, smem)
-        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, strided_tma_kernel<A, B, 1, false>, nthreads, smem);
+        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, strided_tma_kernel<A, B, -1, 0>, nthreads, smem)
+        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, strided_tma_kernel<A, B, 1, 0>, nthreads, smem);
     return e == cudaSuccess ? n : 0;
   }
   static int zconv_blocks_per_sm(int nthreads, size_t smem) {
@@ -736,12 +805,13 @@ struct LaunchTma {
     if (a.grid <= 0) return cudaSuccess;
     const size_t smem = strided_smem(a.T, a.boxr, a.nbox, a.nst);
     using K = void (*)(const StridedTmaArgs);
-    const bool ts = a.tensor_store && a.T * A <= a.nthreads;
-    K k = dir < 0 ? (ts ? (K)strided_tma_kernel<A, B, -1, true> : (K)strided_tma_kernel<A, B, -1, false>)
-                  : (ts ? (K)strided_tma_kernel<A, B, 1, true> : (K)strided_tma_kernel<A, B, 1, false>);
+    const bool pair = a.pair && (a.line_len % 2 == 0) && (a.T % 2 == 0);
+    const bool ts = !pair && a.tensor_store && a.T * A <= a.nthreads;
+    K k = dir < 0 ? (pair ? (K)strided_tma_kernel<A, B, -1, 2> : ts ? (K)strided_tma_kernel<A, B, -1, 1> : (K)strided_tma_kernel<A, B, -1, 0>)
+                  : (pair ? (K)strided_tma_kernel<A, B, 1, 2> : ts ? (K)strided_tma_kernel<A, B, 1, 1> : (K)strided_tma_kernel<A, B, 1, 0>);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)a.grid);
-    cfg.blockDim = dim3((unsigned)a.nthreads);
+    cfg.blockDim = dim3((unsigned)(pair ? strided_tma_pair_threads<A, B>() : a.nthreads));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = s;
     cudaLaunchAttribute at[1];
