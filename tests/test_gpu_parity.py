@@ -822,3 +822,38 @@ def test_blocked_config2_size_shares_back_projectors(mvd, config2):
     ref = O.deconvolve_blocked(config2.views, config2.psfs, block[::-1], "osem", 3)
     check(got.cpu().numpy(), ref, 3, "blocked config 2")
     assert launches > 8 * 3 * 3 * 8
+
+
+# ------------------------------------------------------------------------------------------
+# seeded random small problems: odd / even / prime extents (rows that are not 16-byte aligned, ragged tiles, PSF
+# boxes larger than the volume), every variant and kernel mode, with and without weights, Tikhonov, graph replay
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("case", range(16))
+def test_random_small_problems(mvd, case):
+    import torch
+    rng = np.random.default_rng([13080730, 900, case])
+    dims = tuple(int(rng.integers(5, 72)) for _ in range(3))                     # (Nx, Ny, Nz)
+    box = tuple(int(2 * rng.integers(1, 6) + 1) for _ in range(3))               # odd 3..11
+    V = int(rng.integers(1, 5))
+    variant = ("osem", "efficient", "independent")[int(rng.integers(3))]
+    mode = ("auto", "plain", "compound", "opt1", "opt2")[int(rng.integers(5))]
+    lam = float(rng.choice([0.0, 0.0, 0.006, 0.06]))
+    use_w = variant == "osem" and bool(rng.integers(2))
+    use_graph = bool(rng.integers(2))
+    iters = int(rng.integers(1, 4))
+    p = mvd_synth.make_tiny_asymmetric(dims=dims, psf_dims=box, n_views=V, seed_stream=50 + case)
+    kw, okw = {}, {}
+    if lam:
+        kw["tikhonov_lambda"] = okw["tikhonov_lambda"] = lam
+    if use_w:
+        ws = [rng.random(p.views[0].shape).astype(np.float32) for _ in range(V)]
+        kw["weights"] = [torch.from_numpy(w).cuda() for w in ws]
+        okw["weights"] = [w.astype(np.float64) for w in ws]
+    if use_graph:
+        kw["use_graph"] = True
+    g, st = gpu_checkpoints(mvd, p, variant, mode, (1, iters) if iters > 1 else (1,), **kw)
+    o, orc = oracle_checkpoints(p, variant, mode, (1, iters) if iters > 1 else (1,), **okw)
+    what = "case %d: dims %s box %s V=%d %s/%s lam=%g w=%s graph=%s" % (case, dims, box, V, variant, mode, lam, use_w, use_graph)
+    check(g[1], o[1], 1, what)
+    check(g[iters], o[iters], iters, what)
+    assert st["flux"] == pytest.approx(orc.flux, rel=1e-5), what
