@@ -152,3 +152,34 @@ def test_no_gpu_means_a_loud_failure(lib):
     import numpy as np
     with pytest.raises(mvd.MvdError):
         mvd.Deconvolver([torch.zeros(8, 8, 8)], [np.ones((3, 3, 3), np.float32)])
+
+
+def test_planner_on_random_problems(lib):
+    """Host planner, seeded sweep: for any volume and (odd) PSF boxes the FFT lengths are supported lengths (2-3-5-7-
+    smooth, x even), alias-free (M >= N + r, x half row: M >= ceil(Nx/2) + 2 r_x, and M >= K), never wasteful beyond the
+    spacing of the length table, and the workspace covers what the layout needs."""
+    import numpy as np
+    rng = np.random.default_rng(20130807)
+    for _ in range(300):
+        dims = tuple(int(rng.integers(1, 1100)) for _ in range(3))
+        V = int(rng.integers(1, 5))
+        boxes = [tuple(int(2 * rng.integers(0, 32) + 1) for _ in range(3)) for _ in range(V)]
+        r = [max((b[a] - 1) // 2 for b in boxes) for a in range(3)]
+        need = ((dims[0] + 1) // 2 + 2 * r[0], max(dims[1] + r[1], 2 * r[1] + 1), max(dims[2] + r[2], 2 * r[2] + 1))
+        if max(need) > 1296:
+            assert mvd.workspace_size(dims, boxes, "osem") == 0          # no length that long: refused, not mis-planned
+            continue
+        m = mvd.plan_dims(dims, boxes)
+        assert m[0] % 2 == 0
+        for a in range(3):
+            assert m[a] >= need[a], (dims, boxes, m)
+            n = m[a]
+            for p in (2, 3, 5, 7):
+                while n % p == 0:
+                    n //= p
+            assert n == 1
+            assert m[a] <= max(need[a] * 1.16, need[a] + 8), (dims, boxes, m)
+        ws = mvd.workspace_size(dims, boxes, "osem")
+        nvox = dims[0] * dims[1] * dims[2]
+        assert ws >= 2 * V * m[0] * m[1] * m[2] * 8 + m[0] * m[1] * dims[2] * 8 + 2 * 4 * nvox
+        assert mvd.workspace_size(dims, boxes, "efficient") >= ws + m[0] * m[1] * dims[2] * 8

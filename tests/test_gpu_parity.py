@@ -770,6 +770,23 @@ def test_register_staged_fallback_kernels_match_too(mvd, tiny, monkeypatch):
         check(g[3], o[3], 3, "fallback %s" % variant)
 
 
+def test_experiment_knobs_keep_parity(mvd, tiny, monkeypatch):
+    """The documented tuning / experiment knobs select other kernels or schedules, never other results: plain loads
+    of the real rows, the 8 x 2 z tile, tensor stores and column pairs in the y pass, cluster pacing, z-chunked
+    schedule.  Same parity bar; the z-chunked schedule is bit-identical to the default."""
+    ref, _ = gpu_checkpoints(mvd, tiny, "osem", "auto", (3,))
+    o, _ = oracle_checkpoints(tiny, "osem", "auto", (3,))
+    for knobs in ({"MVD_XBULK": "0"}, {"MVD_ZTX": "8"}, {"MVD_YTSTORE": "1"}, {"MVD_YPAIR": "1"},
+                  {"MVD_YCLUSTER": "2", "MVD_ZCLUSTER": "2"}, {"MVD_ZCHUNK": "5"}):
+        for k, v in knobs.items():
+            monkeypatch.setenv(k, v)
+        g, _ = gpu_checkpoints(mvd, tiny, "osem", "auto", (3,), use_graph=True)
+        check(g[3], o[3], 3, str(knobs))
+        assert np.array_equal(g[3], ref[3]), knobs          # same arithmetic per element in every variant
+        for k in knobs:
+            monkeypatch.delenv(k)
+
+
 def test_views_not_16_byte_aligned(mvd):
     """Borrowed views (and weights) only need float alignment: rows that cannot be staged by 16-byte
     bulk copies take the plain-load path inside the same kernel."""
