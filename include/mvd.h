@@ -153,6 +153,36 @@ MVD_API size_t mvd_reduce_scratch_bytes(void);
 MVD_API mvd_status mvd_reduce_sum(const float* src_device, long long n, void* scratch_device, void* stream,
                                   double* host_out);
 
+/* mvd_reduce_sum for callers that cannot supply scratch memory (same quantity: the sum of n device floats in fp64,
+ * the numerator of the initial estimate psi^0 = mean of the views, PAPER.md L304 / L421).
+ *
+ * Every other call of this library works in memory the caller hands over, and mvd_reduce_sum is no exception: it
+ * needs a scratch buffer.  Some callers have none to give and cannot allocate one: a job whose workspace already
+ * fills the GPU (config 5 whole takes ~150 of 180 GB) or whose memory pool took all of HBM at start-up, so that
+ * cudaMalloc fails; a time-lapse loop that sums every new time-point while other streams upload the next, where one
+ * cudaMalloc/cudaFree pair per time-point would synchronise the device and undo the overlap; a plug-in of a host
+ * application that receives device pointers but may not allocate on that application's GPU.  This call keeps its
+ * partial sums in a fixed array compiled into the library's device image instead: about 128 KB on every GPU that
+ * loads libmvd.so, held until the process exits.  It calls no cudaMalloc, cudaFree or allocating routine.
+ *
+ *   src_device  n floats on the CURRENT device (borrowed, read-only; any alignment); stream must belong to it.
+ *   n           0 <= n <= mvd_reduce_sum_static_max() = 2^30 floats (one partial per 65536 floats, 16384 partials).
+ *               Larger n: MVD_ERR_UNSUPPORTED, nothing is launched; split the input and add the pieces, or use
+ *               mvd_reduce_sum.  n < 0 or a NULL pointer: MVD_ERR_INVALID_ARG.  CUDA failure: MVD_ERR_CUDA.
+ *   host_out    HOST address of the result; the stream is synchronised before the call returns.
+ *   mvd_reduce_sum_static_error(): the reason for the calling thread's last failure, "" after a success.
+ * The result is the same for every launch and every GPU (fixed chunks, partials added in index order); it equals
+ * mvd_reduce_sum's up to the rounding order of the fp64 additions (relative difference ~1e-15).
+ * Set-up: the first call on each device looks up the array's device address (with that device current) and keeps it;
+ * make that first call before any stream capture begins on that device.
+ * Sharing: all calls on a device use the one array, which still holds the previous call's partials; the call clears
+ * the one word that has to start at zero by itself.  Two calls whose GPU work overlaps (two streams, two host
+ * threads) race on the array and return garbage: issue them one after the other (each call synchronises its stream
+ * before it returns, so back-to-back calls from one thread are safe). */
+MVD_API long long mvd_reduce_sum_static_max(void);
+MVD_API const char* mvd_reduce_sum_static_error(void);
+MVD_API mvd_status mvd_reduce_sum_static(const float* src_device, long long n, void* stream, double* host_out);
+
 /* Builds a context: normalises the PSFs, computes the back-projectors K_v on the device (eq. 105 /
  * 107 / 108), their spectra and those of P_v, and the initial estimate.  Synchronises the stream
  * before returning.  See the header comment for pointer kinds and ownership. */

@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     MvdError,
     ViewParallelDeconvolver,
     reduce_sum,
+    reduce_sum_static,
     split_views,
     deconvolve_blocked,
     load_library,

@@ -26,6 +26,7 @@ SYMBOLS = (
     "mvd_launch_count", "mvd_profile", "mvd_profile_read", "mvd_kernel_class_name", "mvd_blocked_workspace_size", "mvd_deconvolve_blocked", "mvd_destroy",
     "mvd_status_string", "mvd_last_error",
     "mvd_compare", "mvd_partial_product", "mvd_get_product", "mvd_apply_product", "mvd_reduce_scratch_bytes", "mvd_reduce_sum",
+    "mvd_reduce_sum_static", "mvd_reduce_sum_static_max", "mvd_reduce_sum_static_error",
 )
 
 
@@ -126,6 +127,12 @@ def load_library():
     lib.mvd_reduce_scratch_bytes.restype = C.c_size_t
     lib.mvd_reduce_sum.argtypes = [vp, C.c_longlong, vp, vp, C.POINTER(C.c_double)]
     lib.mvd_reduce_sum.restype = C.c_int
+    lib.mvd_reduce_sum_static.argtypes = [vp, C.c_longlong, vp, C.POINTER(C.c_double)]
+    lib.mvd_reduce_sum_static.restype = C.c_int
+    lib.mvd_reduce_sum_static_max.argtypes = []
+    lib.mvd_reduce_sum_static_max.restype = C.c_longlong
+    lib.mvd_reduce_sum_static_error.argtypes = []
+    lib.mvd_reduce_sum_static_error.restype = C.c_char_p
     _lib = lib
     return lib
 
@@ -449,6 +456,32 @@ def reduce_sum(t, stream=None):
     with torch.cuda.device(t.device):
         _check(lib.mvd_reduce_sum(t.data_ptr(), t.numel(), scratch.data_ptr(), stream.cuda_stream, C.byref(out)),
                None, "mvd_reduce_sum")
+    return float(out.value)
+
+
+def reduce_sum_static(t, stream=None):
+    """mvd_reduce_sum_static: the same fp64 sum as reduce_sum, for callers that must not allocate.
+
+    reduce_sum asks torch for a scratch tensor on every call.  A job whose workspace already fills the GPU, a time-lapse
+    loop that cannot afford the allocator's device-wide synchronisation between time-points, or an embedding
+    application that forbids allocations on its device cannot do that; this call allocates nothing, neither here nor in
+    the library: the partial sums go to a fixed ~128 KB array inside libmvd.so's device image (include/mvd.h has the
+    details).  Hence the rules: `t` is used where it lies (a non-contiguous tensor is refused rather than copied), at most
+    2^30 elements (MvdError beyond that), and two calls whose GPU work could overlap must not be issued concurrently.
+    The first call on a device also looks up the array's address; make it before capturing any stream of that device.
+    """
+    import torch
+    lib = load_library()
+    if t.dtype != torch.float32 or not t.is_cuda or not t.is_contiguous():
+        raise MvdError("reduce_sum_static: needs a contiguous float32 CUDA tensor (no copy is made: that would allocate)")
+    stream = stream if stream is not None else torch.cuda.current_stream(t.device)
+    stream.wait_stream(torch.cuda.current_stream(t.device))
+    out = C.c_double(0.0)
+    with torch.cuda.device(t.device):
+        st = lib.mvd_reduce_sum_static(t.data_ptr(), t.numel(), stream.cuda_stream, C.byref(out))
+    if st != 0:
+        raise MvdError("mvd_reduce_sum_static: %s (%s)" % (lib.mvd_status_string(st).decode(),
+                                                           lib.mvd_reduce_sum_static_error().decode()))
     return float(out.value)
 
 

@@ -2,7 +2,7 @@
 
     python -m paper_1308_0730_b200.build [-j N] [--force]
 
-One object per supported pencil length (csrc/lengths.def x csrc/inst.cu) plus csrc/mvd.cu, compiled
+One object per supported pencil length (csrc/lengths.def x csrc/inst.cu) plus csrc/mvd.cu and csrc/reduce_static.cu, compiled
 in parallel, cached by modification time under csrc/build/<hash of the compiler flags>/ (so objects of an
 experiment build are never linked into a normal one), linked into
 paper_1308_0730_b200/libmvd.so.  Nothing here runs at import time of the package.
@@ -71,11 +71,12 @@ def build(jobs=None, force=False, verbose=True):
             tasks.append([NVCC, *FLAGS, "-DMVD_INST_A=%d" % a, "-DMVD_INST_B=%d" % b, "-c", src, "-o", o])
     host_deps = hdr[4:] + [os.path.join(CSRC, f) for f in ("mvd.cu", "misc_kernels.cuh", "lengths.def")] + \
         [os.path.join(os.path.dirname(HERE), "include", "mvd.h")]
-    for name in ("mvd",):
+    # reduce_static.cu is self-contained (the no-allocation sum with its file-scope device array): it depends on mvd.h only
+    for name, deps in (("mvd", host_deps), ("reduce_static", [os.path.join(CSRC, "reduce_static.cu"), host_deps[-1]])):
         o = os.path.join(OBJ, name + ".o")
         objs.append(o)
         src = os.path.join(CSRC, name + ".cu")
-        if force or _newer(o, [d for d in host_deps if os.path.exists(d)]):
+        if force or _newer(o, [d for d in deps if os.path.exists(d)]):
             tasks.append([NVCC, *FLAGS, "-c", src, "-o", o])
     jobs = jobs or max(1, len(os.sched_getaffinity(0)))
     if verbose:
