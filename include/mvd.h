@@ -145,7 +145,8 @@ MVD_API mvd_status mvd_compare(mvd_ctx* ctx, const float* ref_device, double* av
  *                         counts as one iteration.  Every rank applies the same product, so psi stays replicated.
  * MVD_INDEPENDENT / MVD_EFFICIENT only (MVD_ERR_UNSUPPORTED for MVD_OSEM: sequential updates do not split).
  * mvd_reduce_sum: sum of n device floats in fp64 -> *host_out (for the global mean of the views); scratch = DEVICE
- * memory of at least mvd_reduce_scratch_bytes(). */
+ * memory of at least mvd_reduce_scratch_bytes() on the device of src (a constant of the build: it does not depend on
+ * which device is current when it is asked for). */
 MVD_API mvd_status mvd_partial_product(mvd_ctx* ctx);
 MVD_API mvd_status mvd_get_product(mvd_ctx* ctx, float** acc_device);
 MVD_API mvd_status mvd_apply_product(mvd_ctx* ctx, int total_views);

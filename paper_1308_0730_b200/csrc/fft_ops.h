@@ -21,9 +21,7 @@ __host__ __device__ constexpr int strided_tma_tile(int M) { return (M > 500 && M
 //      elements x the whole pencil, loaded by tensor copies with zero fill beyond n_in ----------
 struct StridedTmaArgs {
   CUtensorMap in_map;      // dims (x: line_len, pencil: n_in, outer: n_outer); box (T, boxr, 1)
-  CUtensorMap out_map;     // tensor_store: dims (x: line_len, pencil: n_out, outer: n_outer); same box
   int pair;                // 1: two adjacent columns per thread, 128-bit accesses (needs even line_len and T)
-  int tensor_store;        // 1: results go back into the staged tile and leave by tensor copies (rows >= n_out clipped)
   float2* out;
   const float2* tw;        // tw[j] = exp(-2*pi*i*j/M)
   int T, nthreads, grid;
@@ -35,7 +33,6 @@ struct StridedTmaArgs {
   int n_out;               // pencil outputs >= n_out are not stored
   int reverse;             // walk the tiles last to first (reads what the previous pass wrote last: L2 hits)
   int nst;                 // shared-memory stages of the tile: 1 or 2
-  int cluster;             // > 1: launched as clusters of this many CTAs that pace their prefetches together
 };
 
 // ---- TMA-staged fused z pass: input tile and spectrum tile by tensor copies --------------------
@@ -52,7 +49,6 @@ struct ZconvTmaArgs {
   long long plane;         // elements between z planes of `out`
   int nz;                  // planes written
   int nst_in;              // shared-memory stages of the input tile: 1 or 2
-  int cluster;             // > 1: clusters of this many CTAs pace their prefetches together
 };
 
 // ---- strided pencil FFT (y pass, plain z pass): pencils along a strided axis, tiles of T
@@ -145,10 +141,10 @@ struct LengthOps {
   int (*xrow_tma_flags)(const XArgs&, int mode);   // compile-time variant of the kernel this launch selects
   cudaError_t (*strided_tma)(const StridedTmaArgs&, int dir, cudaStream_t);
   size_t (*strided_tma_smem)(int T, int boxr, int nbox, int nst);
-  int (*strided_tma_blocks_per_sm)(int dir, int nthreads, size_t smem);
+  int (*strided_tma_blocks_per_sm)(const StridedTmaArgs&, int dir);   // resident CTAs per SM of the kernel this launch selects
   cudaError_t (*zconv_tma)(const ZconvTmaArgs&, cudaStream_t);
   size_t (*zconv_tma_smem)(int T, int boxr, int nbox, int nst_in);
-  int (*zconv_tma_blocks_per_sm)(int nthreads, size_t smem);
+  int (*zconv_tma_blocks_per_sm)(const ZconvTmaArgs&);
 };
 
 // table of all compiled lengths, ascending in M

@@ -154,12 +154,41 @@ static int reduce_blocks() { return 8 * sm_count(); }
 // combined variants: the running product of the f_v is kept in fp32; beyond this many views every factor takes the
 // |V|-th root before it enters the product (same value, no overflow or underflow for any V the ABI accepts)
 constexpr int kRootEachViews = 16;
-constexpr int kMaxZChunks = 64;   // z-chunked schedule: at most this many chunks (one statistics slot each)
 
-static int env_int(const char* name, int dflt) {
-  const char* s = getenv(name);
-  return (s && *s) ? atoi(s) : dflt;
-}
+// Tuning / comparison knobs: ONE environment variable, read once per plan and once per context,
+//   MVD_TUNE="key=value,key=value,..."   (integer values; unknown keys are ignored)
+// Every knob selects another kernel or tile shape, never another result (tests/test_gpu_parity.py runs them against
+// the oracle).  Keys: xtma ytma ztma (0: register-staged fallback kernels of pass_kernels.cuh), rxt xt_smem_kb
+// (rows / shared-memory cap of an x tile), ynst znst (tile stages of the y / z pass), ztx (8: z tile of 8 x by 2 rows),
+// ypair (0/1: column pairs in the y pass; default on from 1000-point pencils), xbulk (0: real rows by plain loads),
+// flip (0: no alternating tile order), corr_tiled (0: untiled precompute correlation), and for the fallback
+// kernels ty tz rx xthreads.
+struct Tune {
+  static constexpr int kMax = 24;
+  char key[kMax][16];
+  int val[kMax];
+  int n = 0;
+  Tune() {
+    const char* s = getenv("MVD_TUNE");
+    while (s && *s && n < kMax) {
+      const char* eq = strchr(s, '=');
+      const char* end = strchr(s, ',');
+      if (!end) end = s + strlen(s);
+      if (eq && eq < end && eq - s > 0 && eq - s < 16) {
+        memcpy(key[n], s, (size_t)(eq - s));
+        key[n][eq - s] = 0;
+        val[n] = atoi(eq + 1);
+        ++n;
+      }
+      s = *end ? end + 1 : end;
+    }
+  }
+  int get(const char* k, int dflt) const {
+    for (int i = 0; i < n; ++i)
+      if (strcmp(key[i], k) == 0) return val[i];
+    return dflt;
+  }
+};
 
 // tile width for a strided pass over a contiguous extent L; single_round: T*max(A,B) <= max_threads
 static void choose_tile(const LengthOps* l, long long L, bool single_round, int force, int* T_out,
@@ -229,14 +258,15 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
   P.wsize = P.plane * P.N[2];
   P.ssize = P.plane * P.Mz;
 
-  choose_tile(P.ly, P.Mx, false, env_int("MVD_TY", 0), &P.Ty, &P.nty);
-  choose_tile(P.lz, P.plane, true, env_int("MVD_TZ", 0), &P.Tz, &P.ntz);
+  const Tune tune;
+  choose_tile(P.ly, P.Mx, false, tune.get("ty", 0), &P.Ty, &P.nty);
+  choose_tile(P.lz, P.plane, true, tune.get("tz", 0), &P.Tz, &P.ntz);
   choose_tile(P.lz, P.plane, false, 0, &P.Tzs, &P.ntzs);
   choose_tile(P.ly, P.Mx, false, 0, &P.Tys, &P.ntys);
   {
     const int ab = std::max(P.lx->A, P.lx->B);
-    int R = std::max(1, env_int("MVD_XTHREADS", 256) / ab);
-    const int force = env_int("MVD_RX", 0);
+    int R = std::max(1, tune.get("xthreads", 256) / ab);
+    const int force = tune.get("rx", 0);
     if (force > 0) R = force;
     R = std::min(R, std::max(1, P.lx->max_threads / ab));
     while (R > 1 && P.lx->xrow_smem(R, P.r[0]) > 160 * 1024) --R;
@@ -249,58 +279,45 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
 
   {
     // TMA-staged y and z passes: tile widths are multiples of 4 (16-byte rows, 128-byte boxes)
-    auto plan_tma = [&](const LengthOps* l, int L, int force, size_t smem_cap, bool zconv, int* T_out,
-                        int* nt_out, int* box_out, int* nbox_out) {
+    auto plan_tma = [&](const LengthOps* l, bool zconv, int* T_out, int* nt_out, int* box_out, int* nbox_out) {
       const int ab = std::max(l->A, l->B);
       const int nbox = (l->M + 255) / 256;
       const int boxr = ((l->M + nbox - 1) / nbox + 3) / 4 * 4;
-      int best = 0;
-      double best_score = -1.0;
-      const int cand[] = {kTmaTileHost};   // the kernels are compiled for one tile width
-      for (int T : cand) {
-        const size_t smem = zconv ? l->zconv_tma_smem(T, boxr, nbox, P.znst) : l->strided_tma_smem(T, boxr, nbox, P.ynst);
-        if (smem > smem_cap && T > 4) continue;
-        const double eff = double(L) / double(((L + T - 1) / T) * T);
-        const double seg = T >= 8 ? 1.0 : 0.7;
-        if (eff * seg > best_score + 1e-9) { best_score = eff * seg; best = T; }
-      }
-      if (best == 0) best = 4;
-      (void)force;
-      best = zconv ? kTmaTileHost : strided_tma_tile(l->M);
-      const int items = best * ab * (zconv ? 2 : 1);   // the z tile is 8 x by 2 rows
+      const int T = zconv ? kTmaTileHost : strided_tma_tile(l->M);   // the kernels are compiled for one tile width
+      const int items = T * ab * (zconv ? 2 : 1);   // the z tile is 16 columns
       const int rounds = (items + l->max_threads - 1) / l->max_threads;
-      *T_out = best;
+      *T_out = T;
       *nt_out = std::min(l->max_threads, round_up32((items + rounds - 1) / rounds));
       *box_out = boxr;
       *nbox_out = nbox;
-      const size_t smem = zconv ? l->zconv_tma_smem(best, boxr, nbox, P.znst) : l->strided_tma_smem(best, boxr, nbox, P.ynst);
+      const size_t smem = zconv ? l->zconv_tma_smem(T, boxr, nbox, P.znst) : l->strided_tma_smem(T, boxr, nbox, P.ynst);
       return smem <= 220 * 1024;
     };
-    P.znst = env_int("MVD_ZNST", 2) == 1 ? 1 : 2;
+    P.znst = tune.get("znst", 2) == 1 ? 1 : 2;
     {
       // two tile stages whenever they fit (one stage with more CTAs per SM measured slower on config 5)
       const int nbox = (P.ly->M + 255) / 256;
       const int boxr = ((P.ly->M + nbox - 1) / nbox + 3) / 4 * 4;
       P.ynst = P.ly->strided_tma_smem(strided_tma_tile(P.ly->M), boxr, nbox, 2) <= 218 * 1024 ? 2 : 1;
-      const int force = env_int("MVD_YNST", 0);
+      const int force = tune.get("ynst", 0);
       if (force == 1 || force == 2) P.ynst = force;
       const int nbz = (P.lz->M + 255) / 256;
       const int bxz = ((P.lz->M + nbz - 1) / nbz + 3) / 4 * 4;
-      if (env_int("MVD_ZNST", 0) == 0) P.znst = P.lz->zconv_tma_smem(kTmaTileHost, bxz, nbz, 2) <= 218 * 1024 ? 2 : 1;
+      if (tune.get("znst", 0) == 0) P.znst = P.lz->zconv_tma_smem(kTmaTileHost, bxz, nbz, 2) <= 218 * 1024 ? 2 : 1;
     }
-    P.ytma = env_int("MVD_YTMA", 1);
-    P.ztma = env_int("MVD_ZTMA", 1);
-    if (!plan_tma(P.ly, P.Mx, 0, (size_t)env_int("MVD_YT_SMEM_KB", 72) * 1024, false, &P.Tyt, &P.ntyt, &P.ybox, &P.ynbox)) P.ytma = 0;
-    if (!plan_tma(P.lz, P.Mx, 0, (size_t)env_int("MVD_ZT_SMEM_KB", 110) * 1024, true, &P.Tzt, &P.ntzt, &P.zbox, &P.znbox)) P.ztma = 0;
+    P.ytma = tune.get("ytma", 1);
+    P.ztma = tune.get("ztma", 1);
+    if (!plan_tma(P.ly, false, &P.Tyt, &P.ntyt, &P.ybox, &P.ynbox)) P.ytma = 0;
+    if (!plan_tma(P.lz, true, &P.Tzt, &P.ntzt, &P.zbox, &P.znbox)) P.ztma = 0;
   }
   {
     // TMA-staged x pass (quotient / OSEM update): rows per tile sized for >= 3 resident CTAs per SM
     const int ab = std::max(P.lx->A, P.lx->B);
-    P.xtma = env_int("MVD_XTMA", 1);
+    P.xtma = tune.get("xtma", 1);
     int R = std::max(1, 160 / ab);   // kXrowTmaThreads of pass_tma.cuh
-    const int force = env_int("MVD_RXT", 0);
+    const int force = tune.get("rxt", 0);
     // 45 KB: five CTAs per SM; larger radices hold fewer CTAs (registers), so they get larger tiles
-    const size_t cap = (size_t)env_int("MVD_XT_SMEM_KB", ab <= 21 ? 45 : (ab <= 28 ? 72 : 100)) * 1024;
+    const size_t cap = (size_t)tune.get("xt_smem_kb", ab <= 21 ? 45 : (ab <= 28 ? 72 : 100)) * 1024;
     while (R > 1 && P.lx->xrow_tma_smem(R, P.r[0], P.N[0], P.weighted) > cap) --R;
     if (force > 0 && force * ab <= 160 && P.lx->xrow_tma_smem(force, P.r[0], P.N[0], P.weighted) <= 220 * 1024) R = force;
     if (P.lx->xrow_tma_smem(R, P.r[0], P.N[0], P.weighted) > 220 * 1024) P.xtma = 0;
@@ -340,7 +357,7 @@ static mvd_status make_plan(Plan& P, int n_views, const int dims[3], const int (
   P.off_kern = take(P.psf_stride * sizeof(double) * P.V);
   P.off_auto = take(kmode == MVD_KERNEL_COMPOUND ? P.auto_stride * sizeof(double) * P.V : 256);
   P.sum_blocks = reduce_blocks();
-  P.off_partials = take(sizeof(double) * 2 * (size_t)std::max(P.nctax, P.sum_blocks * kMaxZChunks));
+  P.off_partials = take(sizeof(double) * 2 * (size_t)std::max(P.nctax, P.sum_blocks));
   P.off_scalars = take(sizeof(double) * (size_t)(P.V + 8));
   P.off_cmp = take(sizeof(double) * (6 * 192 + 8));   // mvd_compare partials
   P.total = o;
@@ -361,7 +378,8 @@ struct mvd_ctx {
   float eps = 1e-6f, psi_floor = 1e-6f, tikhonov = 0.f;
   cudaStream_t stream = nullptr;
   char* ws = nullptr;
-  char* psf_staging = nullptr;   // pinned, device-mapped host copy of the PSF taps; lives for the duration of mvd_create
+  char* psf_staging = nullptr;   // pinned, device-mapped host copy of the PSF taps (process-wide buffer, held under its lock)
+  cudaEvent_t staged_read = nullptr;   // recorded behind the last kernel that reads psf_staging
   std::vector<const float*> views;
   std::vector<const float*> weights;   // empty or one per view (borrowed)
   std::vector<char> is_local;          // view-parallel contexts: which views this context owns (all by default)
@@ -369,17 +387,11 @@ struct mvd_ctx {
   float psi0_value = 0.f;
   const float* psi0_ptr = nullptr;     // options.psi0 (borrowed), for mvd_restart
   bool w_valid = false;        // the work buffer holds the x-forward transform of the current psi
-                               // (z-chunked schedule: the x- and y-forward transform)
   int y_pair = 0;              // y pass: two columns per thread, 128-bit shared-memory and global accesses
                                // (MVD_YPAIR=0/1; default: on for pencils of 1000 points or more)
-  int y_tensor_store = 0;      // y pass: results leave by tensor copies from the staged tile instead of per-thread stores
-  int ycluster = 1;            // CTAs per cluster of the TMA-staged y pass (1 = plain launch)
-  int zcluster = 1;            // ... of the TMA-staged z pass
   int corr_tiled = 1;          // 0: the untiled fp64 correlation kernel of the precompute (MVD_CORR_TILED=0)
   int xbulk = 1;               // 0: real rows of the x pass by plain loads (MVD_XBULK=0, for comparison)
   int ztx = 16;                // z pass tile: 16 x of one row (default), or 8 x of two rows y
-  int zchunk = 0;              // > 0: the plane-local passes (y-inverse, x pass, y-forward) run chunk by chunk of this
-                               // many z planes, so a chunk of the work buffer stays in L2 between them
   bool broken = false;
   bool stats_valid = false;
   int stats_ncta = 0;
@@ -394,8 +406,8 @@ struct mvd_ctx {
   int xt_blocks[5][4] = {};          // resident CTAs per SM of the TMA-staged x pass, per (mode, compile-time flags)
   int flip = 0;                      // tile direction of the next x / y launch (alternates: L2 reuse)
   int use_flip = 1;
-  int yt_blocks[2] = {0, 0};         // ... of the TMA-staged y pass (forward, inverse)
-  int zt_blocks = 0;                 // ... of the TMA-staged z pass
+  int yt_blocks[2][2] = {};          // ... of the TMA-staged y pass, per (direction, column-pair variant)
+  int zt_blocks[2] = {0, 0};         // ... of the TMA-staged z pass, per tile shape (8 x 2, 16 x 1)
   // per-kernel-class event timing (mvd_profile)
   bool profiling = false;
   std::vector<cudaEvent_t> ev_pool;
@@ -499,28 +511,17 @@ mvd_status y_pass_tma(mvd_ctx* c, float2* buf, int dir, int nz_planes, int xt0, 
     return MVD_ERR_CUDA;
   }
   a.out = buf; a.tw = c->twy();
-  a.tensor_store = c->y_tensor_store;
   a.pair = c->y_pair;
-  if (a.tensor_store && !make_map3(&a.out_map, buf, P.Mx, dir < 0 ? P.My : P.N[1], nz_planes, P.Mx, P.plane, P.Tyt, P.ybox, 1)) {
-    snprintf(c->err, sizeof(c->err), "y pass: cuTensorMapEncodeTiled failed");
-    c->broken = true;
-    return MVD_ERR_CUDA;
-  }
   a.T = P.Tyt; a.nthreads = P.ntyt; a.boxr = P.ybox; a.nbox = P.ynbox;
   a.xt0 = xt0; a.n_xt = n_xt; a.nst = P.ynst;
   a.line_len = P.Mx; a.n_outer = nz_planes;
   a.out_outer_stride = P.plane; a.out_pstride = P.Mx;
   a.n_out = dir < 0 ? P.My : P.N[1];
   a.reverse = c->use_flip ? (c->flip ^= 1) : 0;
-  int& bl = c->yt_blocks[dir < 0 ? 0 : 1];
-  if (bl == 0) bl = P.ly->strided_tma_blocks_per_sm(dir, a.nthreads, P.ly->strided_tma_smem(a.T, a.boxr, a.nbox, a.nst));
+  int& bl = c->yt_blocks[dir < 0 ? 0 : 1][a.pair ? 1 : 0];
+  if (bl == 0) bl = P.ly->strided_tma_blocks_per_sm(a, dir);
   if (bl <= 0) { snprintf(c->err, sizeof(c->err), "y pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
   a.grid = (int)std::min<long long>((long long)n_xt * nz_planes, (long long)c->num_sms * bl);
-  a.cluster = c->ycluster;
-  if (a.cluster > 1) {
-    a.grid = a.grid / a.cluster * a.cluster;
-    if (a.grid == 0) { a.grid = 1; a.cluster = 1; }
-  }
   {
     ProfScope ps(c, dir < 0 ? MVD_K_Y_FWD : MVD_K_Y_INV);
     MVD_CK(P.ly->strided_tma(a, dir, c->stream), "y pass (TMA)");
@@ -544,14 +545,10 @@ mvd_status z_conv_tma(mvd_ctx* c, const float2* in, float2* out, const float2* s
   a.T = P.Tzt; a.nthreads = P.ntzt; a.boxr = P.zbox; a.nbox = P.znbox;
   a.xt0 = xt0; a.n_xt = n_xt; a.tx = tx;
   a.mx = P.Mx; a.my = P.My; a.plane = P.plane; a.nz = P.N[2]; a.nst_in = P.znst;
-  if (c->zt_blocks == 0) c->zt_blocks = P.lz->zconv_tma_blocks_per_sm(a.nthreads, P.lz->zconv_tma_smem(a.T, a.boxr, a.nbox, a.nst_in));
-  if (c->zt_blocks <= 0) { snprintf(c->err, sizeof(c->err), "z pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
-  a.grid = (int)std::min<long long>((long long)n_xt * ((P.My + ty - 1) / ty), (long long)c->num_sms * c->zt_blocks);
-  a.cluster = c->zcluster;
-  if (a.cluster > 1) {
-    a.grid = a.grid / a.cluster * a.cluster;
-    if (a.grid == 0) { a.grid = 1; a.cluster = 1; }
-  }
+  int& bl = c->zt_blocks[tx == 16 ? 1 : 0];
+  if (bl == 0) bl = P.lz->zconv_tma_blocks_per_sm(a);
+  if (bl <= 0) { snprintf(c->err, sizeof(c->err), "z pass: kernel does not fit on an SM"); c->broken = true; return MVD_ERR_CUDA; }
+  a.grid = (int)std::min<long long>((long long)n_xt * ((P.My + ty - 1) / ty), (long long)c->num_sms * bl);
   {
     ProfScope ps(c, MVD_K_Z_CONV);
     MVD_CK(P.lz->zconv_tma(a, c->stream), "z convolution pass (TMA)");
@@ -688,51 +685,9 @@ mvd_status conv_core(mvd_ctx* c, const float2* in, float2* buf, const float2* sp
   return MVD_OK;
 }
 
-// y-inverse -> x pass (quotient or update) -> y-forward of planes [z0, z0 + nz): all three are local to a z plane
-mvd_status plane_group(mvd_ctx* c, int v, bool update, int z0, int nz, int chunk_index) {
-  const Plan& P = c->P;
-  const int rx = (P.K[v].x - 1) / 2;
-  float2* w = c->W() + (long long)z0 * P.plane;
-  const long long voff = (long long)z0 * P.N[1] * P.N[0];
-  MVD_TRY(y_pass(c, w, +1, nz, false));
-  XArgs a = x_args(c, w, w, rx);
-  a.nrows = (long long)P.N[1] * nz;
-  a.psi = c->psi() + voff;
-  a.partials = c->partials() + 2 * (size_t)chunk_index * P.sum_blocks;
-  if (!update) {
-    a.phi = c->views[v] + voff;
-    MVD_TRY(x_pass(c, a, X_QUOT));
-  } else {
-    a.wts = c->weights.empty() ? nullptr : c->weights[v] + voff;
-    MVD_TRY(x_pass(c, a, a.wts ? X_UPDATE_W : X_UPDATE));
-  }
-  MVD_TRY(y_pass(c, w, -1, nz, false));
-  return MVD_OK;
-}
-
 // one iteration (every view contributes once, L817); requires w_valid
 mvd_status iteration_body(mvd_ctx* c) {
   const Plan& P = c->P;
-  if (!P.combined && c->zchunk > 0) {
-    // eq. 109-112 with the plane-local passes chunked along z: per view  z(H), [y-inv, quotient, y-fwd] per chunk,
-    // z(K), [y-inv, update, y-fwd] per chunk; the work buffer enters and leaves x- and y-transformed
-    const int nchunks = (P.N[2] + c->zchunk - 1) / c->zchunk;
-    for (int v = 0; v < P.V; ++v) {
-      for (int half = 0; half < 2; ++half) {
-        MVD_TRY(z_conv(c, c->W(), c->W(), half ? c->specK(v) : c->specH(v)));
-        if (half == 1 && v == P.V - 1)   // statistics of the last update: one slot of sum_blocks partials per chunk
-          MVD_CK(cudaMemsetAsync(c->partials(), 0, sizeof(double) * 2 * (size_t)nchunks * P.sum_blocks, c->stream), "memset partials");
-        for (int k = 0; k < nchunks; ++k) {
-          // alternate the chunk order so a pass starts on the planes the z pass / previous group wrote last
-          const int kk = (half & 1) ? nchunks - 1 - k : k;
-          const int z0 = kk * c->zchunk, nz = std::min(c->zchunk, P.N[2] - z0);
-          MVD_TRY(plane_group(c, v, half == 1, z0, nz, kk));
-        }
-      }
-    }
-    c->stats_ncta = nchunks * P.sum_blocks;
-    return MVD_OK;
-  }
   if (!P.combined) {
     // eq. 109-112: psi updated after every view, index order (R11)
     for (int v = 0; v < P.V; ++v) {
@@ -767,7 +722,6 @@ mvd_status iteration_body(mvd_ctx* c) {
 mvd_status ensure_w(mvd_ctx* c) {
   if (c->w_valid) return MVD_OK;
   MVD_TRY(x_load(c, c->psi(), c->P.combined ? c->W0() : c->W()));
-  if (!c->P.combined && c->zchunk > 0) MVD_TRY(y_pass(c, c->W(), -1, c->P.N[2], false));
   c->w_valid = true;
   return MVD_OK;
 }
@@ -863,7 +817,8 @@ mvd_status precompute(mvd_ctx* c, const float* const* psfs_host, const double* s
     for (int v = 0; v < P.V; ++v) total += align_up((size_t)P.K[v].x * P.K[v].y * P.K[v].z * sizeof(float), 256);
     // one grow-only pinned buffer per process, handed from one mvd_create to the next (allocating and freeing
     // mapped pinned memory per context cost tens of milliseconds now and then: the block-wise mode creates a context
-    // per block shape); held under a lock until this mvd_create has synchronised its stream
+    // per block shape); held under a lock until the last normalise kernel has read it (event below), so that
+    // concurrent mvd_create calls of per-GPU threads serialise on this short section only
     c->psf_staging = staging_acquire(total);
     if (!c->psf_staging) { snprintf(c->err, sizeof(c->err), "pinned PSF staging: allocation failed"); return MVD_ERR_CUDA; }
     char* dev_base = nullptr;
@@ -885,6 +840,8 @@ mvd_status precompute(mvd_ctx* c, const float* const* psfs_host, const double* s
       ++c->launches;
       off += align_up(sizeof(float) * n, 256);
     }
+    MVD_CK(cudaEventCreateWithFlags(&c->staged_read, cudaEventDisableTiming), "staging event");
+    MVD_CK(cudaEventRecord(c->staged_read, c->stream), "staging event");
   }
   // back-projectors K_v (O3)
   if (shared_kern) {
@@ -1066,19 +1023,15 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
   c->stream = reinterpret_cast<cudaStream_t>(opt->stream);
   c->ws = reinterpret_cast<char*>(opt->workspace);
   c->use_graph = opt->use_graph;
-  c->use_flip = env_int("MVD_FLIP", 1);
-  c->y_tensor_store = env_int("MVD_YTSTORE", 0) ? 1 : 0;
+  const Tune tune;
+  c->use_flip = tune.get("flip", 1);
   {   // measured: 1050-point pencils (one CTA per SM) 937 -> 887 us per launch; 525-point pencils 110 -> 112 us
-    const int yp = env_int("MVD_YPAIR", -1);
+    const int yp = tune.get("ypair", -1);
     c->y_pair = yp < 0 ? (c->P.My >= 1000 ? 1 : 0) : (yp ? 1 : 0);
   }
-  c->ycluster = std::min(8, std::max(1, env_int("MVD_YCLUSTER", 1)));
-  c->zcluster = std::min(8, std::max(1, env_int("MVD_ZCLUSTER", 1)));
-  c->corr_tiled = env_int("MVD_CORR_TILED", 1);
-  c->xbulk = env_int("MVD_XBULK", 1);
-  c->ztx = env_int("MVD_ZTX", 16) == 8 ? 8 : 16;   // 16 x 1 measured faster than 8 x 2 on configs 2-5
-  c->zchunk = std::max(0, env_int("MVD_ZCHUNK", 0));
-  if (c->zchunk > 0) c->zchunk = std::max(c->zchunk, (c->P.N[2] + kMaxZChunks - 1) / kMaxZChunks);
+  c->corr_tiled = tune.get("corr_tiled", 1);
+  c->xbulk = tune.get("xbulk", 1);
+  c->ztx = tune.get("ztx", 16) == 8 ? 8 : 16;   // 16 x 1 measured faster than 8 x 2 on configs 2-5
   if (c->use_graph && !c->stream) {   // the legacy default stream cannot be captured
     fprintf(stderr, "mvd_create: use_graph needs a non-default stream\n");
     delete c;
@@ -1110,17 +1063,20 @@ static mvd_status create_impl(mvd_ctx** out, int n_views, const float* const* vi
   }
 
   s = precompute(c, psfs, shared_kern);
+  if (c->psf_staging) {
+    // the kernels that read the staged taps are the first of the precompute: normally long done by now.
+    // No event (an early failure) -> wait for the whole stream
+    if (!c->staged_read || cudaEventSynchronize(c->staged_read) != cudaSuccess) cudaStreamSynchronize(c->stream);
+    staging_release();
+    c->psf_staging = nullptr;
+  }
+  if (c->staged_read) { cudaEventDestroy(c->staged_read); c->staged_read = nullptr; }
   if (s == MVD_OK && opt->views_ready &&
       c->fail(cudaStreamWaitEvent(c->stream, reinterpret_cast<cudaEvent_t>(opt->views_ready), 0), "views_ready"))
     s = MVD_ERR_CUDA;
   c->psi0_ptr = opt->psi0;
   if (s == MVD_OK) s = init_estimate(c, opt->psi0);
   if (s == MVD_OK && c->fail(cudaStreamSynchronize(c->stream), "mvd_create")) s = MVD_ERR_CUDA;
-  if (c->psf_staging) {
-    if (s != MVD_OK) cudaStreamSynchronize(c->stream);   // a kernel may still be reading the staged taps
-    staging_release();
-    c->psf_staging = nullptr;
-  }
   if (s != MVD_OK) {
     if (c->err[0]) fprintf(stderr, "mvd_create: %s\n", c->err);
     delete c;
@@ -1248,13 +1204,15 @@ mvd_status mvd_apply_product(mvd_ctx* c, int total_views) {
   return MVD_OK;
 }
 
-size_t mvd_reduce_scratch_bytes(void) { return sizeof(double) * (size_t)(mvd::reduce_blocks() + 8); }
+// the scratch layout does not depend on the device that happens to be current: kMaxReduceBlocks partials + the total
+static constexpr int kMaxReduceBlocks = 2048;
+size_t mvd_reduce_scratch_bytes(void) { return sizeof(double) * (size_t)(kMaxReduceBlocks + 8); }
 
 mvd_status mvd_reduce_sum(const float* src, long long n, void* scratch, void* stream, double* host_out) {
   if (!src || n < 0 || !scratch || !host_out) return MVD_ERR_INVALID_ARG;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   double* part = reinterpret_cast<double*>(scratch);
-  const int nb = mvd::reduce_blocks();
+  const int nb = std::min(mvd::reduce_blocks(), kMaxReduceBlocks);
   sum_f32_kernel<<<nb, 256, 0, st>>>(src, n, part);
   if (cudaGetLastError() != cudaSuccess) return MVD_ERR_CUDA;
   final_sum_kernel<<<1, 256, 0, st>>>(part, nb, 1, part + nb);

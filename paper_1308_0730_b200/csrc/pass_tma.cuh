@@ -89,7 +89,12 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
   const unsigned mis_r = shifted ? (unsigned)((reinterpret_cast<uintptr_t>(real_src) >> 2) & 3u) : 0u;
   const unsigned mis_w = (shifted && has_w) ? (unsigned)((reinterpret_cast<uintptr_t>(p.wts) >> 2) & 3u) : 0u;
   auto row_shift = [&](unsigned mis, int g) { return (int)((mis + (unsigned)g * (unsigned)p.nx) & 3u); };
-  auto row_staged = [&](int a, int g) { return (g > 0 || a == 0) && (g < nrows_i - 1 || ((a + p.nx) & 3) == 0); };
+  // a row is staged by a bulk copy only if its whole 16-byte-aligned window [g*nx - a, g*nx - a + roundup4(a + nx))
+  // lies inside the array (for nx >= 3 that excludes at most the first and the last row; shorter rows: a few more)
+  auto row_staged = [&](int a, int g) {
+    const long long lo = (long long)g * p.nx - a, hi = lo + ((a + p.nx + 3) & ~3);
+    return lo >= 0 && hi <= (long long)nrows_i * p.nx;
+  };
 
   if (tid == 0) {
     mbar_init(&bars[0], 1);   // complex rows landed
@@ -298,6 +303,9 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
         });
       }
     }
+    // rows that could not be staged were written into rst / wrst by ordinary stores; the copy engine (async proxy)
+    // refills those slots next
+    if (shifted) fence_proxy_async();
     __syncthreads();
     // every read of the real rows is done: stage the next tile's
     if (tid < 32 && more && real_bulk) issue_r(tile + (int)gridDim.x);
@@ -357,32 +365,17 @@ __global__ void __launch_bounds__(kXrowTmaThreads, xrow_min_blocks(PassCfg<A, B>
 //   stage 1: item (n2, x) owns rows n1*B + n2 -> A-point FFT, twiddle -> rows k1*B + n2
 //   stage 2: item (k1, x) owns rows k1*B + n2 -> B-point FFT -> global rows k1 + A*k2 (< n_out)
 // =========================================================================================
-// TS: the stage-2 results are written back into the staged tile (after every item has read its inputs) and leave
-// by tensor copies (SASS UTMASTG) instead of per-thread stores; needs a single round of stage-2 items per tile.
-// threads the planner gives the y pass of this length (one round of items per stage when they fit)
-template <int A, int B>
-constexpr int strided_tma_threads() {
-  constexpr int items = strided_tma_tile(A * B) * PassCfg<A, B>::AB_MAX;
-  constexpr int rounds = (items + PassCfg<A, B>::MAX_THREADS - 1) / PassCfg<A, B>::MAX_THREADS;
-  constexpr int t = ((items + rounds - 1) / rounds + 31) / 32 * 32;
-  return t < PassCfg<A, B>::MAX_THREADS ? t : PassCfg<A, B>::MAX_THREADS;
-}
-
-// VAR: 0 = per-thread stores, 1 = TS (tensor stores, above), 2 = PAIR: a thread transforms two adjacent columns at once,
-// so every shared-memory and global access is 128 bits wide (half the load / store / address instructions, half the
-// threads, twice the independent work per thread).
+// PAIR: a thread transforms two adjacent columns at once, so every shared-memory and global access is 128 bits wide
+// (half the load / store / address instructions, half the threads, twice the independent work per thread).
 template <int A, int B>
 constexpr int strided_tma_pair_threads() {
   constexpr int items = strided_tma_tile(A * B) / 2 * PassCfg<A, B>::AB_MAX;
   constexpr int t = (items + 31) / 32 * 32;
   return t < 512 ? t : 512;
 }
-template <int A, int B, int DIR, int VAR>
-__global__ void __launch_bounds__(VAR == 1 ? strided_tma_threads<A, B>() : (VAR == 2 ? strided_tma_pair_threads<A, B>() : PassCfg<A, B>::MAX_THREADS),
-                                  VAR == 1 ? 2 : 0)
+template <int A, int B, int DIR, bool PAIR>
+__global__ void __launch_bounds__(PAIR ? strided_tma_pair_threads<A, B>() : PassCfg<A, B>::MAX_THREADS)
 strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
-  constexpr bool TS = VAR == 1;
-  constexpr bool PAIR = VAR == 2;
   constexpr int M = A * B;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int T = strided_tma_tile(M);
@@ -414,21 +407,13 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
 
   if (tid == 0 && (int)blockIdx.x < ntiles) issue((int)blockIdx.x, 0);
 
-  // p.cluster > 1: the CTAs of a cluster take adjacent x tiles and meet at a cluster barrier before every prefetch,
-  // so the copies of one memory row (cluster * T contiguous elements) are issued together
-  const int rounds = p.cluster > 1 ? (ntiles + (int)gridDim.x - 1) / (int)gridDim.x : 0;
   int it = 0;
-  for (int tile = blockIdx.x; p.cluster > 1 ? it < rounds : tile < ntiles; tile += gridDim.x, ++it) {
-    if (p.cluster > 1) {
-      cluster_arrive_wait();
-      if (tile >= ntiles) continue;
-    }
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
     const int s = nst == 2 ? (it & 1) : 0;
     float2* sm = buf + (size_t)s * NR * T;
     const bool more = tile + (int)gridDim.x < ntiles;
-    // tensor stores: the other stage is still being read by the previous tile's store; its refill waits until
-    // after stage 1 of this tile
-    if (tid == 0 && more && nst == 2 && !TS) issue(tile + (int)gridDim.x, s ^ 1);
+    // two stages: the other stage was last read before the final barrier of the previous tile
+    if (tid == 0 && more && nst == 2) issue(tile + (int)gridDim.x, s ^ 1);
     const int rtile = p.reverse ? ntiles - 1 - tile : tile;
     const int outer = rtile / p.n_xt;
     const int x0 = (p.xt0 + (rtile - outer * p.n_xt)) * T;
@@ -479,42 +464,7 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
       }
     }
     __syncthreads();
-    if constexpr (TS) {
-      if (tid == 0 && more && nst == 2) {
-        bulk_wait_read0();                       // the previous tile's store has read the other stage
-        issue(tile + (int)gridDim.x, s ^ 1);
-      }
-      const int j = tid;                         // one round: T * A <= blockDim.x (checked by the host)
-      const int k1 = j / T;
-      const int x = j - k1 * T;
-      const bool act = j < T * A;
-      float2 u[B];
-      if (act) {
-        static_for<0, B>([&](auto n2_) {
-          constexpr int n2 = decltype(n2_)::value;
-          u[n2] = sm[(k1 * B + n2) * T + x];
-        });
-        FftReg<B, DIR>::run(u);
-      }
-      __syncthreads();                           // every input of the tile has been read
-      if (act) {
-        static_for<0, B>([&](auto k2_) {
-          constexpr int k2 = decltype(k2_)::value;
-          sm[(k1 + A * k2) * T + x] = u[k2];
-        });
-      }
-      fence_proxy_async();                       // generic-proxy stores -> visible to the copy engine
-      __syncthreads();
-      if (tid == 0) {
-        for (int b = 0; b < p.nbox; ++b)
-          if (b * p.boxr < p.n_out) tma_store_3d(&p.out_map, sm + (size_t)(b * p.boxr) * T, x0, b * p.boxr, outer);
-        bulk_commit();
-        if (more && nst == 1) {
-          bulk_wait_read0();
-          issue(tile + (int)gridDim.x, 0);
-        }
-      }
-    } else if constexpr (PAIR) {
+    if constexpr (PAIR) {
       constexpr int H = T / 2;
       const float4* sm4 = reinterpret_cast<const float4*>(sm);
       float2* out = p.out + (long long)outer * p.out_outer_stride + x0;
@@ -567,9 +517,6 @@ strided_tma_kernel(const __grid_constant__ StridedTmaArgs p) {
       __syncthreads();   // every read of this tile is done
       if (tid == 0 && more && nst == 1) issue(tile + (int)gridDim.x, 0);   // one stage: refill it now
     }
-  }
-  if constexpr (TS) {
-    if (tid == 0) bulk_wait_read0();             // shared memory must outlive the last store's reads
   }
 }
 
@@ -630,13 +577,8 @@ zconv_tma_kernel(const __grid_constant__ ZconvTmaArgs p) {
     issue_spec((int)blockIdx.x);
   }
 
-  const int rounds = p.cluster > 1 ? (ntiles + (int)gridDim.x - 1) / (int)gridDim.x : 0;   // see strided_tma_kernel
   int it = 0;
-  for (int tile = blockIdx.x; p.cluster > 1 ? it < rounds : tile < ntiles; tile += gridDim.x, ++it) {
-    if (p.cluster > 1) {
-      cluster_arrive_wait();
-      if (tile >= ntiles) continue;
-    }
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
     const int s = nst == 2 ? (it & 1) : 0;
     float2* sm = buf + (size_t)s * NR * T;
     const float2* sp = sbuf;
@@ -744,12 +686,10 @@ struct LaunchTma {
     MVD_SET((xrow_tma_kernel<A, B, X_ACCUM, 0>));
     MVD_SET((xrow_tma_kernel<A, B, X_ACCUM, XF_LAST>));
     MVD_SET((xrow_tma_kernel<A, B, X_ACCUM, XF_LAST | XF_TIK>));
-    MVD_SET((strided_tma_kernel<A, B, -1, 0>));
-    MVD_SET((strided_tma_kernel<A, B, 1, 0>));
-    MVD_SET((strided_tma_kernel<A, B, -1, 1>));
-    MVD_SET((strided_tma_kernel<A, B, 1, 1>));
-    MVD_SET((strided_tma_kernel<A, B, -1, 2>));
-    MVD_SET((strided_tma_kernel<A, B, 1, 2>));
+    MVD_SET((strided_tma_kernel<A, B, -1, false>));
+    MVD_SET((strided_tma_kernel<A, B, 1, false>));
+    MVD_SET((strided_tma_kernel<A, B, -1, true>));
+    MVD_SET((strided_tma_kernel<A, B, 1, true>));
     MVD_SET((zconv_tma_kernel<A, B, 8>));
     MVD_SET((zconv_tma_kernel<A, B, 16>));
 #undef MVD_SET
@@ -789,59 +729,36 @@ struct LaunchTma {
   static size_t zconv_smem(int T, int boxr, int nbox, int nst_in) {   // T = 8 x 2 rows = 16 columns
     return (size_t)(nst_in + 1) * boxr * nbox * 2 * T * sizeof(float2) + (size_t)B * Cfg::AP * sizeof(float2) + 32;
   }
-  static int strided_blocks_per_sm(int dir, int nthreads, size_t smem) {
+  // the kernel a launch with these arguments selects, and its block size: the occupancy query and the launch agree
+  using SKernel = void (*)(const StridedTmaArgs);
+  static bool strided_pair(const StridedTmaArgs& a) { return a.pair && (a.line_len % 2 == 0) && (a.T % 2 == 0); }
+  static SKernel strided_kernel_of(int dir, bool pair) {
+    return dir < 0 ? (pair ? (SKernel)strided_tma_kernel<A, B, -1, true> : (SKernel)strided_tma_kernel<A, B, -1, false>)
+                   : (pair ? (SKernel)strided_tma_kernel<A, B, 1, true> : (SKernel)strided_tma_kernel<A, B, 1, false>);
+  }
+  static int strided_threads(const StridedTmaArgs& a) { return strided_pair(a) ? strided_tma_pair_threads<A, B>() : a.nthreads; }
+  static int strided_blocks_per_sm(const StridedTmaArgs& a, int dir) {
     int n = 0;
-    cudaError_t e = dir < 0
-        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, strided_tma_kernel<A, B, -1, 0>, nthreads, smem)
-        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, strided_tma_kernel<A, B, 1, 0>, nthreads, smem);
+    const cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+        &n, strided_kernel_of(dir, strided_pair(a)), strided_threads(a), strided_smem(a.T, a.boxr, a.nbox, a.nst));
     return e == cudaSuccess ? n : 0;
   }
-  static int zconv_blocks_per_sm(int nthreads, size_t smem) {
+  static int zconv_blocks_per_sm(const ZconvTmaArgs& a) {
     int n = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, zconv_tma_kernel<A, B, 8>, nthreads, smem);
+    const size_t smem = zconv_smem(a.T, a.boxr, a.nbox, a.nst_in);
+    const cudaError_t e = a.tx == 16 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, zconv_tma_kernel<A, B, 16>, a.nthreads, smem)
+                                     : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, zconv_tma_kernel<A, B, 8>, a.nthreads, smem);
     return e == cudaSuccess ? n : 0;
   }
   static cudaError_t strided(const StridedTmaArgs& a, int dir, cudaStream_t s) {
     if (a.grid <= 0) return cudaSuccess;
     const size_t smem = strided_smem(a.T, a.boxr, a.nbox, a.nst);
-    using K = void (*)(const StridedTmaArgs);
-    const bool pair = a.pair && (a.line_len % 2 == 0) && (a.T % 2 == 0);
-    const bool ts = !pair && a.tensor_store && a.T * A <= a.nthreads;
-    K k = dir < 0 ? (pair ? (K)strided_tma_kernel<A, B, -1, 2> : ts ? (K)strided_tma_kernel<A, B, -1, 1> : (K)strided_tma_kernel<A, B, -1, 0>)
-                  : (pair ? (K)strided_tma_kernel<A, B, 1, 2> : ts ? (K)strided_tma_kernel<A, B, 1, 1> : (K)strided_tma_kernel<A, B, 1, 0>);
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)a.grid);
-    cfg.blockDim = dim3((unsigned)(pair ? strided_tma_pair_threads<A, B>() : a.nthreads));
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = s;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = (unsigned)std::max(1, a.cluster);
-    at[0].val.clusterDim.y = 1;
-    at[0].val.clusterDim.z = 1;
-    cfg.attrs = at;
-    cfg.numAttrs = a.cluster > 1 ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, k, a);
+    strided_kernel_of(dir, strided_pair(a))<<<a.grid, strided_threads(a), smem, s>>>(a);
+    return cudaGetLastError();
   }
   static cudaError_t zconv(const ZconvTmaArgs& a, cudaStream_t s) {
     if (a.grid <= 0) return cudaSuccess;
     const size_t smem = zconv_smem(a.T, a.boxr, a.nbox, a.nst_in);
-    if (a.cluster > 1) {
-      cudaLaunchConfig_t cfg = {};
-      cfg.gridDim = dim3((unsigned)a.grid);
-      cfg.blockDim = dim3((unsigned)a.nthreads);
-      cfg.dynamicSmemBytes = smem;
-      cfg.stream = s;
-      cudaLaunchAttribute at[1];
-      at[0].id = cudaLaunchAttributeClusterDimension;
-      at[0].val.clusterDim.x = (unsigned)a.cluster;
-      at[0].val.clusterDim.y = 1;
-      at[0].val.clusterDim.z = 1;
-      cfg.attrs = at;
-      cfg.numAttrs = 1;
-      return a.tx == 16 ? cudaLaunchKernelEx(&cfg, zconv_tma_kernel<A, B, 16>, a)
-                        : cudaLaunchKernelEx(&cfg, zconv_tma_kernel<A, B, 8>, a);
-    }
     if (a.tx == 16) zconv_tma_kernel<A, B, 16><<<a.grid, a.nthreads, smem, s>>>(a);
     else zconv_tma_kernel<A, B, 8><<<a.grid, a.nthreads, smem, s>>>(a);
     return cudaGetLastError();

@@ -760,9 +760,8 @@ def test_every_compiled_length_on_every_axis(mvd, axis):
 
 def test_register_staged_fallback_kernels_match_too(mvd, tiny, monkeypatch):
     """The register-staged passes (pass_kernels.cuh) stay as the fallback when a pencil does not fit
-    the TMA-staged tiles; MVD_XTMA/YTMA/ZTMA=0 selects them.  Same parity bar."""
-    for k in ("MVD_XTMA", "MVD_YTMA", "MVD_ZTMA"):
-        monkeypatch.setenv(k, "0")
+    the TMA-staged tiles; MVD_TUNE="xtma=0,ytma=0,ztma=0" selects them.  Same parity bar."""
+    monkeypatch.setenv("MVD_TUNE", "xtma=0,ytma=0,ztma=0")
     for variant in ("osem", "efficient"):
         g, _ = gpu_checkpoints(mvd, tiny, variant, "auto", (1, 3))
         o, _ = oracle_checkpoints(tiny, variant, "auto", (1, 3))
@@ -770,21 +769,18 @@ def test_register_staged_fallback_kernels_match_too(mvd, tiny, monkeypatch):
         check(g[3], o[3], 3, "fallback %s" % variant)
 
 
-def test_experiment_knobs_keep_parity(mvd, tiny, monkeypatch):
-    """The documented tuning / experiment knobs select other kernels or schedules, never other results: plain loads
-    of the real rows, the 8 x 2 z tile, tensor stores and column pairs in the y pass, cluster pacing, z-chunked
-    schedule.  Same parity bar; the z-chunked schedule is bit-identical to the default."""
+def test_tuning_knobs_keep_parity(mvd, tiny, monkeypatch):
+    """The keys of MVD_TUNE (csrc/mvd.cu) select other kernels or tile shapes, never other results: plain loads of the
+    real rows, the 8 x 2 z tile, column pairs in the y pass, one tile stage, no alternating tile order, and several at
+    once.  Same parity bar, and bit-identical to the default: every variant does the same arithmetic per element."""
     ref, _ = gpu_checkpoints(mvd, tiny, "osem", "auto", (3,))
     o, _ = oracle_checkpoints(tiny, "osem", "auto", (3,))
-    for knobs in ({"MVD_XBULK": "0"}, {"MVD_ZTX": "8"}, {"MVD_YTSTORE": "1"}, {"MVD_YPAIR": "1"},
-                  {"MVD_YCLUSTER": "2", "MVD_ZCLUSTER": "2"}, {"MVD_ZCHUNK": "5"}):
-        for k, v in knobs.items():
-            monkeypatch.setenv(k, v)
+    for knobs in ("xbulk=0", "ztx=8", "ypair=1", "ynst=1,znst=1", "flip=0", "ypair=1,ztx=8,xbulk=0,rxt=2", "nosuchkey=3"):
+        monkeypatch.setenv("MVD_TUNE", knobs)
         g, _ = gpu_checkpoints(mvd, tiny, "osem", "auto", (3,), use_graph=True)
-        check(g[3], o[3], 3, str(knobs))
-        assert np.array_equal(g[3], ref[3]), knobs          # same arithmetic per element in every variant
-        for k in knobs:
-            monkeypatch.delenv(k)
+        check(g[3], o[3], 3, knobs)
+        assert np.array_equal(g[3], ref[3]), knobs
+    monkeypatch.delenv("MVD_TUNE")
 
 
 def test_views_not_16_byte_aligned(mvd):
