@@ -136,3 +136,25 @@ def test_config5_whole_volume_combined_variants_on_sub_volumes(mvd, config5, var
         o.iterate(2)
         ref = o.psi[z0 - cz0:z0 - cz0 + S, y0 - cy0:y0 - cy0 + S, x0 - cx0:x0 - cx0 + S]
         check(g[z0:z0 + S, y0:y0 + S, x0:x0 + S], ref, 2, "config 5 %s, sub-volume at %s" % (variant, (z0, y0, x0)))
+
+
+# The PSF-size sweep of BASELINE configs[4] (9^3 ... 31x31x63; a larger PSF means a larger effective
+# block overhead): bench.py --psf-sweep times these boxes, this test is their parity.  The views are config-5-recipe
+# draws on a 128x128x96 volume the oracle finishes in seconds; the PSFs are the sweep's own recipe
+# (sigma_xy = r_x / 4, sigma_z = r_z / 3.5, the config's view angles).  All three variants, two iterations.
+@pytest.mark.parametrize("box", [(9, 9, 9), (13, 13, 27), (31, 31, 63)])
+def test_psf_sweep_boxes_match_the_oracle(mvd, box):
+    prob = mvd_synth.make_problem(5, n_views=3, dims=(128, 128, 96), psf_dims=box)
+    sxy, sz = max((box[0] - 1) / 2 / 4.0, 0.5), max((box[2] - 1) / 2 / 3.5, 0.5)
+    psfs = [mvd_synth.gaussian_psf(box, sxy, sz, a) for a in mvd_synth.CONFIGS[5]["angles"][:3]]
+    views = to_dev(prob.views)
+    for variant in ("osem", "efficient", "independent"):
+        d = mvd.Deconvolver(views, psfs, variant=variant)
+        o = O.Oracle(prob.views, psfs, variant)
+        for it in (1, 2):
+            d.iterate(1)
+            o.iterate(1)
+            check(d.get_estimate_host(), o.psi, it, "sweep box %s %s" % (box, variant))
+        st = d.get_stats()
+        assert abs(st["flux"] - o.psi.sum()) <= 1e-5 * o.psi.sum()
+        d.close()
